@@ -1,0 +1,124 @@
+"""ctypes access to the CPU oracle (oracle/los_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs; never by paper_2509_25110_b200/.  Two builds of the same
+C file: `f64` (REAL = double, the fp64 oracle and the timed CPU baseline) and `f80`
+(REAL = x87 long double, the grading reference of reading R14).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "los_oracle.c")
+_FLAGS = ["-O2", "-std=c11", "-fno-fast-math", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared"]
+_LOCK = threading.Lock()
+_LIBS: dict[str, ctypes.CDLL] = {}
+
+_pd = ctypes.POINTER(ctypes.c_double)
+_pi = ctypes.POINTER(ctypes.c_int32)
+
+
+def lib_path(real: str) -> str:
+    return os.path.join(_HERE, f"liblos_oracle_{real}.so")
+
+
+def build(force: bool = False) -> None:
+    """Compile both oracle builds with gcc (a few seconds)."""
+    for real, defs in (("f64", []), ("f80", ["-DORACLE_LONG_DOUBLE"])):
+        out = lib_path(real)
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+            continue
+        tmp = f"{out}.{os.getpid()}.tmp"
+        subprocess.run(["gcc", *_FLAGS, *defs, _SRC, "-o", tmp, "-lm"], check=True)
+        os.replace(tmp, out)
+
+
+def _lib(real: str) -> ctypes.CDLL:
+    if real not in ("f64", "f80"):
+        raise ValueError("real must be 'f64' or 'f80'")
+    with _LOCK:
+        if real not in _LIBS:
+            build()
+            lib = ctypes.CDLL(lib_path(real))
+            lib.oracle_real_mant_bits.restype = ctypes.c_int
+            lib.oracle_lcut.argtypes = [ctypes.c_double]
+            lib.oracle_lcut.restype = ctypes.c_int
+            lib.oracle_sph_bessel.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_trapz_weights.argtypes = [_pd, ctypes.c_int, _pd]
+            lib.oracle_transfer.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
+                                            ctypes.c_double, _pd, _pd, _pd, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_cls.argtypes = [ctypes.c_int, ctypes.c_int, _pd, ctypes.c_int, _pd, _pd,
+                                       ctypes.c_int, _pd]
+            assert lib.oracle_real_mant_bits() == (53 if real == "f64" else 64)
+            _LIBS[real] = lib
+        return _LIBS[real]
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(_pd)
+
+
+DEFAULT_MARGIN = 30
+
+
+def lcut(x: float) -> int:
+    return _lib("f64").oracle_lcut(float(x))
+
+
+def sph_bessel(x: float, lmax: int, margin: int = DEFAULT_MARGIN, real: str = "f64") -> np.ndarray:
+    """j_l(x), l = 0..lmax."""
+    out = np.empty(lmax + 1, dtype=np.float64)
+    if _lib(real).oracle_sph_bessel(float(x), int(lmax), int(margin), _ptr(out)):
+        raise ValueError("oracle_sph_bessel: bad arguments")
+    return out
+
+
+def trapz_weights(t, real: str = "f64") -> np.ndarray:
+    t = _f64(t)
+    w = np.empty_like(t)
+    if _lib(real).oracle_trapz_weights(_ptr(t), t.size, _ptr(w)):
+        raise ValueError("oracle_trapz_weights: bad arguments")
+    return w
+
+
+def transfer(l_list, k, tau, tau0, S_T, S_E, S_phi=None, margin: int = DEFAULT_MARGIN,
+             real: str = "f64", nthreads: int = 0) -> np.ndarray:
+    """Delta[n_src][n_l][n_k] (Eq. 2-3)."""
+    l_list = np.ascontiguousarray(l_list, dtype=np.int32)
+    k, tau, S_T, S_E = _f64(k), _f64(tau), _f64(S_T), _f64(S_E)
+    assert S_T.shape == (k.size, tau.size) and S_E.shape == S_T.shape
+    sp = None
+    if S_phi is not None:
+        S_phi = _f64(S_phi)
+        assert S_phi.shape == S_T.shape
+        sp = _ptr(S_phi)
+    n_src = 3 if S_phi is not None else 2
+    out = np.empty((n_src, l_list.size, k.size), dtype=np.float64)
+    rc = _lib(real).oracle_transfer(l_list.ctypes.data_as(_pi), l_list.size, _ptr(k), k.size,
+                                    _ptr(tau), tau.size, float(tau0), _ptr(S_T), _ptr(S_E), sp,
+                                    int(margin), int(nthreads), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_transfer failed ({rc})")
+    return out
+
+
+def cls(k, Delta, P_R, real: str = "f64", nthreads: int = 0) -> np.ndarray:
+    """C_l[n_spec][n_l] (Eq. 1), order TT, EE, TE, (phiphi)."""
+    k, Delta, P_R = _f64(k), _f64(Delta), _f64(P_R)
+    n_src, n_l, n_k = Delta.shape
+    assert n_k == k.size == P_R.size
+    out = np.empty((3 if n_src == 2 else 4, n_l), dtype=np.float64)
+    rc = _lib(real).oracle_cls(n_src, n_l, _ptr(k), n_k, _ptr(Delta), _ptr(P_R), int(nthreads), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_cls failed ({rc})")
+    return out
