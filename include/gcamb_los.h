@@ -1,0 +1,151 @@
+/*
+ * gcamb_los.h -- C ABI of the B200 (sm_100a) line-of-sight integration library.
+ *
+ * The one data-parallel hot path of gCAMB (arXiv 2509.25110): CAMB's flat-universe
+ * `DoFlatIntegration` inside `SourceToTransfers` (Algorithm 1)
+ * and the C_l assembly of Eq. 1.  "PAPER.md:N" is line N of the paper text; "BJ" is
+ * BASELINE.json `north_star`, which fixes the discrete forms the paper leaves open; "Rn" are
+ * the readings listed in DESIGN.md.
+ *
+ *   Eq. 2  Delta^T_l(k)   = sum_i w_i S_T(k,tau_i)   j_l(x_i)
+ *   Eq. 3  Delta^E_l(k)   = sqrt((l+2)!/(l-2)!) sum_i w_i S_E(k,tau_i) j_l(x_i)/x_i^2
+ *   BJ / PAPER.md:135    Delta^phi_l(k) = sum_i w_i S_phi(k,tau_i) j_l(x_i)
+ *                        x_i = k (tau0 - tau_i), w_i = trapezoid weights of the tau grid (R2)
+ *   Eq. 1  C_l^{XY} = 4 pi sum_j dlnk_j P_R(k_j) Delta^X_l(k_j) Delta^Y_l(k_j)
+ *                        dlnk_j = trapezoid weights of ln k_j (R6); XY = TT, EE, TE, (phiphi) (R12)
+ *
+ * All arithmetic is IEEE fp64.  Every step runs in hand-written CUDA kernels; there is no CPU
+ * fallback.  Pointers are marked HOST or DEVICE.  Device buffers are owned by the caller and
+ * must stay valid until the work enqueued on `cuda_stream` has completed.  `cuda_stream` is a
+ * cudaStream_t cast to void* (NULL = the legacy default stream).
+ *
+ * Threading: a plan is immutable after creation and may be used from several host threads /
+ * streams at once, EXCEPT gcamb_los_spectra_host(), which uses scratch owned by the plan and
+ * must not run concurrently on the same plan.
+ *
+ * Errors: every call returns a gcamb_status; no exception crosses the ABI.  After a non-OK
+ * status gcamb_los_last_error() returns a thread-local message.  NaN/Inf inside S or P_R are
+ * not checked and propagate to the outputs.
+ */
+#ifndef GCAMB_LOS_H
+#define GCAMB_LOS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gcamb_los_plan gcamb_los_plan; /* opaque; owns its device tables */
+
+typedef enum {
+    GCAMB_OK = 0,
+    GCAMB_EINVAL = 1, /* null pointer, size < minimum, l outside [2, 65535], mask/pointer mismatch, n_batch < 1 */
+    GCAMB_EGRID = 2,  /* grid not strictly increasing or not finite, k <= 0, tau_i >= tau0 (x must be > 0, R18) */
+    GCAMB_EALLOC = 3, /* host or device allocation failed */
+    GCAMB_ECUDA = 4   /* any other CUDA error (message in gcamb_los_last_error) */
+} gcamb_status;
+
+/* source mask bits; T and E are mandatory, phi optional (BJ: "TT/EE/TE/phiphi") */
+enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4 };
+
+/*
+ * Plan creation = `IntegrationVars_init` hoisted out of the per-call path:
+ * chi_i = tau0 - tau_i, w_i, dlnk_j, sqrt((l+2)(l+1)l(l-1)), and per (k, tau) point the start
+ * of the downward j_l recurrence: the first l-tile that is not negligible (R16: j_l(x) := 0 for
+ * l above ~ x + 18.2 x^(1/3) + 8, where |j_l| < 1e-36) and the normalised pair
+ * (j_{l+1}(x), j_l(x)) at the top of that tile, generated ON THE DEVICE by Miller's backward
+ * recurrence normalised against closed-form j_0 and j_1 (BJ (b), R15).  That is 20 bytes per
+ * (k, tau) point -- O(N_k N_tau), not an O(N_l N_k N_tau) j_l table.  Also sorts k by cost so
+ * that the heaviest blocks are issued first.
+ *
+ *   l_list  HOST [n_l]   strictly increasing, 2 <= l <= 65535 (any subset; the recurrence walks
+ *                        every l, only listed l are accumulated and stored, R21)
+ *   k       HOST [n_k]   strictly increasing, > 0, finite; n_k >= 2
+ *   tau     HOST [n_tau] strictly increasing, < tau0, finite; n_tau >= 2
+ *   src_mask             GCAMB_SRC_T|GCAMB_SRC_E or GCAMB_SRC_T|GCAMB_SRC_E|GCAMB_SRC_PHI
+ *   cuda_stream          stream the precompute kernels run on; the call synchronises it.
+ * On success *out owns device memory on the CURRENT device; free with gcamb_los_plan_destroy.
+ */
+gcamb_status gcamb_los_plan_create(gcamb_los_plan **out,
+                                   const int32_t *l_list, int32_t n_l,
+                                   const double *k, int32_t n_k,
+                                   const double *tau, int32_t n_tau,
+                                   double tau0, uint32_t src_mask, void *cuda_stream);
+
+/* Frees the plan and its device tables (synchronises the device).  NULL is allowed. */
+gcamb_status gcamb_los_plan_destroy(gcamb_los_plan *plan);
+
+/*
+ * Sizes of a plan.  Any output pointer may be NULL.
+ *   n_src  = 2 (T,E) or 3 (T,E,phi);  n_spec = 3 (TT,EE,TE) or 4 (+phiphi)
+ *   executed_terms = number of (l in l-range, k, tau) triples with l <= min(L(x), l_max), i.e. the
+ *   terms that are not skipped by R16 (the algorithmic work; nominal is n_l*n_k*n_tau).
+ */
+gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32_t *n_k,
+                                 int32_t *n_tau, int32_t *n_src, int32_t *n_spec,
+                                 int64_t *executed_terms);
+
+/*
+ * Eq. 2-3: sources -> transfer functions (steps a1-a3: source staging, j_l recurrence in
+ * registers, tau-integration, cross-thread reduction, Delta^E prefactor).  Asynchronous on
+ * `cuda_stream`; no allocation, no host<->device copy.
+ *   d_S_T, d_S_E, d_S_phi  DEVICE [n_k][n_tau], tau fastest.  d_S_phi must be NULL iff the plan
+ *                          has no GCAMB_SRC_PHI.
+ *   d_Delta                DEVICE [n_src][n_l][n_k], k fastest, order T, E, (phi) -- the
+ *                          (X, l, q) array of PAPER.md:136.  Every element is written.
+ */
+gcamb_status gcamb_los_transfer(const gcamb_los_plan *plan,
+                                const double *d_S_T, const double *d_S_E, const double *d_S_phi,
+                                double *d_Delta, void *cuda_stream);
+
+/*
+ * Eq. 1: transfer functions -> spectra (step a4).  Asynchronous on `cuda_stream`.
+ *   d_Delta DEVICE [n_src][n_l][n_k];  d_P_R DEVICE [n_k];
+ *   d_Cl    DEVICE [n_spec][n_l], order TT, EE, TE, (phiphi).
+ */
+gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_R,
+                           double *d_Cl, void *cuda_stream);
+
+/*
+ * Batched variants (step a5; emulator use-case PAPER.md:24, 248; BJ config 3): n_batch
+ * cosmologies sharing one plan, one launch each.
+ *   d_S_X   DEVICE [n_batch][n_k][n_tau];   d_Delta DEVICE [n_batch][n_src][n_l][n_k]
+ *   d_P_R   DEVICE [n_batch][n_k];          d_Cl    DEVICE [n_batch][n_spec][n_l]
+ */
+gcamb_status gcamb_los_transfer_batched(const gcamb_los_plan *plan, int32_t n_batch,
+                                        const double *d_S_T, const double *d_S_E,
+                                        const double *d_S_phi, double *d_Delta, void *cuda_stream);
+gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
+                                   const double *d_Delta, const double *d_P_R, double *d_Cl,
+                                   void *cuda_stream);
+
+/*
+ * End-to-end convenience with HOST buffers (the paper's "accelerator data region",
+ * PAPER.md:133-136): H2D of the sources and P_R, transfer, cls, D2H of C_l (and of Delta when
+ * h_Delta != NULL), then synchronises `cuda_stream`.  Device scratch is allocated inside the plan
+ * on first use (sized for n_batch) and reused; not thread-safe per plan.  Host buffers should be
+ * pinned for full copy bandwidth but need not be.
+ *   h_S_X HOST [n_batch][n_k][n_tau];  h_P_R HOST [n_batch][n_k];
+ *   h_Cl  HOST [n_batch][n_spec][n_l]; h_Delta HOST [n_batch][n_src][n_l][n_k] or NULL.
+ */
+gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch,
+                                    const double *h_S_T, const double *h_S_E, const double *h_S_phi,
+                                    const double *h_P_R, double *h_Cl, double *h_Delta,
+                                    void *cuda_stream);
+
+/*
+ * Roofline denominator helper: enqueues a pure dependent-chain DFMA kernel (8 independent chains
+ * per thread, `iters` FMAs per chain) on `cuda_stream`.  The caller times it with CUDA events;
+ * it performs exactly  blocks * threads * 8 * iters  DFMAs.  d_out DEVICE [blocks*threads].
+ */
+gcamb_status gcamb_los_dfma_probe(int32_t blocks, int32_t threads, int64_t iters, double *d_out,
+                                  void *cuda_stream);
+
+/* Thread-local message of the last non-OK status on this thread ("" if none). */
+const char *gcamb_los_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GCAMB_LOS_H */

@@ -1,0 +1,267 @@
+// api.cu -- the extern "C" boundary (include/gcamb_los.h): validation, host-side plan tables,
+// launches.  No step of the hot path runs on the host.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "los_internal.cuh"
+
+namespace gcamb {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+gcamb_status cuda_fail(cudaError_t e, const char *what)
+{
+    set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    return e == cudaErrorMemoryAllocation ? GCAMB_EALLOC : GCAMB_ECUDA;
+}
+
+template <class Tp>
+static cudaError_t upload(Tp **dst, const std::vector<Tp> &src, cudaStream_t s)
+{
+    cudaError_t e = cudaMalloc(dst, sizeof(Tp) * src.size());
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyAsync(*dst, src.data(), sizeof(Tp) * src.size(), cudaMemcpyHostToDevice, s);
+}
+
+// composite-trapezoid weights on a non-uniform grid (R2, R6)
+static std::vector<double> trapezoid(const std::vector<double> &t)
+{
+    const size_t n = t.size();
+    std::vector<double> w(n);
+    w[0] = 0.5 * (t[1] - t[0]);
+    for (size_t i = 1; i + 1 < n; ++i) w[i] = 0.5 * (t[i + 1] - t[i - 1]);
+    w[n - 1] = 0.5 * (t[n - 1] - t[n - 2]);
+    return w;
+}
+
+static void free_plan(gcamb_los_plan *p)
+{
+    if (!p) return;
+    cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
+    cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile);
+    cudaFree(p->d_korder);
+    for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
+    cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
+    delete p;
+}
+
+static gcamb_status check_call(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                               const double *S_E, const double *S_phi, const void *out)
+{
+    if (!p || !S_T || !S_E || !out) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    if ((p->n_src == 3) != (S_phi != nullptr)) {
+        set_error("S_phi must be non-NULL exactly when the plan has GCAMB_SRC_PHI");
+        return GCAMB_EINVAL;
+    }
+    return GCAMB_OK;
+}
+
+}  // namespace gcamb
+
+using namespace gcamb;
+
+extern "C" {
+
+const char *gcamb_los_last_error(void) { return g_err; }
+
+gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
+                                   const double *k, int32_t n_k, const double *tau, int32_t n_tau,
+                                   double tau0, uint32_t src_mask, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (!out || !l_list || !k || !tau) { set_error("null argument"); return GCAMB_EINVAL; }
+    if (n_l < 1 || n_k < 2 || n_tau < 2) { set_error("need n_l >= 1, n_k >= 2, n_tau >= 2"); return GCAMB_EINVAL; }
+    if (n_k > 65535) { set_error("n_k must be <= 65535"); return GCAMB_EINVAL; }
+    if (src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
+        set_error("src_mask must be T|E or T|E|PHI");
+        return GCAMB_EINVAL;
+    }
+    for (int i = 0; i < n_l; ++i) {
+        if (l_list[i] < 2 || l_list[i] > 65535) { set_error("l_list[%d] = %d outside [2, 65535]", i, l_list[i]); return GCAMB_EINVAL; }
+        if (i && l_list[i] <= l_list[i - 1]) { set_error("l_list not strictly increasing at %d", i); return GCAMB_EINVAL; }
+    }
+    if (!std::isfinite(tau0)) { set_error("tau0 not finite"); return GCAMB_EGRID; }
+    for (int j = 0; j < n_k; ++j) {
+        if (!std::isfinite(k[j]) || !(k[j] > 0.0)) { set_error("k[%d] must be finite and > 0", j); return GCAMB_EGRID; }
+        if (j && !(k[j] > k[j - 1])) { set_error("k not strictly increasing at %d", j); return GCAMB_EGRID; }
+    }
+    for (int i = 0; i < n_tau; ++i) {
+        if (!std::isfinite(tau[i]) || !(tau[i] < tau0)) { set_error("tau[%d] must be finite and < tau0 (x > 0, R18)", i); return GCAMB_EGRID; }
+        if (i && !(tau[i] > tau[i - 1])) { set_error("tau not strictly increasing at %d", i); return GCAMB_EGRID; }
+    }
+
+    gcamb_los_plan *p = new (std::nothrow) gcamb_los_plan();
+    if (!p) { set_error("out of host memory"); return GCAMB_EALLOC; }
+    std::memset(p, 0, sizeof(*p));
+    p->n_l = n_l; p->n_k = n_k; p->n_tau = n_tau;
+    p->src_mask = src_mask;
+    p->n_src = (src_mask & GCAMB_SRC_PHI) ? 3 : 2;
+    p->n_spec = p->n_src + 1;
+    p->l_min = l_list[0]; p->l_max = l_list[n_l - 1];
+    p->tau0 = tau0;
+    p->shape = choose_shape(n_tau, p->n_src);
+    p->n_tiles = (p->l_max - p->l_min) / p->shape.V + 1;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    // IntegrationVars_init: the O(N) tables, on the host in fp64
+    std::vector<double> vk(k, k + n_k), vtau(tau, tau + n_tau), chi(n_tau), lnk(n_k), pref(n_l);
+    for (int i = 0; i < n_tau; ++i) chi[i] = tau0 - tau[i];
+    for (int j = 0; j < n_k; ++j) lnk[j] = std::log(k[j]);
+    std::vector<double> w = trapezoid(vtau), dlnk = trapezoid(lnk);
+    std::vector<int32_t> l_index((size_t)p->l_max + 1, -1);
+    for (int i = 0; i < n_l; ++i) {
+        const double l = l_list[i];
+        l_index[l_list[i]] = i;
+        pref[i] = std::sqrt((l + 2.0) * (l + 1.0) * l * (l - 1.0));   // (l+2)!/(l-2)!  (R3)
+    }
+
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = upload(&p->d_l_index, l_index, stream);
+    if (e == cudaSuccess) e = upload(&p->d_k, vk, stream);
+    if (e == cudaSuccess) e = upload(&p->d_chi, chi, stream);
+    if (e == cudaSuccess) e = upload(&p->d_w, w, stream);
+    if (e == cudaSuccess) e = upload(&p->d_dlnk, dlnk, stream);
+    if (e == cudaSuccess) e = upload(&p->d_pref, pref, stream);
+    const size_t npt = (size_t)n_k * n_tau;
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_start, sizeof(double2) * npt);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_tile, sizeof(int32_t) * npt);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_korder, sizeof(int32_t) * n_k);
+    // the uploads read pageable vectors that die with this scope
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { gcamb_status st = cuda_fail(e, "plan tables"); free_plan(p); return st; }
+
+    gcamb_status st = plan_precompute(p, stream);
+    if (st != GCAMB_OK) { free_plan(p); return st; }
+    *out = p;
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_plan_destroy(gcamb_los_plan *plan)
+{
+    if (!plan) return GCAMB_OK;
+    cudaError_t e = cudaDeviceSynchronize();
+    free_plan(plan);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceSynchronize");
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32_t *n_k, int32_t *n_tau,
+                                 int32_t *n_src, int32_t *n_spec, int64_t *executed_terms)
+{
+    if (!plan) { set_error("null plan"); return GCAMB_EINVAL; }
+    if (n_l) *n_l = plan->n_l;
+    if (n_k) *n_k = plan->n_k;
+    if (n_tau) *n_tau = plan->n_tau;
+    if (n_src) *n_src = plan->n_src;
+    if (n_spec) *n_spec = plan->n_spec;
+    if (executed_terms) *executed_terms = plan->executed_terms;
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_transfer_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,
+                                        const double *d_S_E, const double *d_S_phi, double *d_Delta,
+                                        void *cuda_stream)
+{
+    gcamb_status st = check_call(plan, n_batch, d_S_T, d_S_E, d_S_phi, d_Delta);
+    if (st != GCAMB_OK) return st;
+    return launch_transfer(plan, n_batch, d_S_T, d_S_E, d_S_phi, d_Delta, (cudaStream_t)cuda_stream);
+}
+
+gcamb_status gcamb_los_transfer(const gcamb_los_plan *plan, const double *d_S_T, const double *d_S_E,
+                                const double *d_S_phi, double *d_Delta, void *cuda_stream)
+{
+    return gcamb_los_transfer_batched(plan, 1, d_S_T, d_S_E, d_S_phi, d_Delta, cuda_stream);
+}
+
+gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Delta,
+                                   const double *d_P_R, double *d_Cl, void *cuda_stream)
+{
+    if (!plan || !d_Delta || !d_P_R || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    return launch_cls(plan, n_batch, d_Delta, d_P_R, d_Cl, (cudaStream_t)cuda_stream);
+}
+
+gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_R,
+                           double *d_Cl, void *cuda_stream)
+{
+    return gcamb_los_cls_batched(plan, 1, d_Delta, d_P_R, d_Cl, cuda_stream);
+}
+
+gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const double *h_S_T,
+                                    const double *h_S_E, const double *h_S_phi, const double *h_P_R,
+                                    double *h_Cl, double *h_Delta, void *cuda_stream)
+{
+    gcamb_status st = check_call(plan, n_batch, h_S_T, h_S_E, h_S_phi, h_Cl);
+    if (st != GCAMB_OK) return st;
+    if (!h_P_R) { set_error("null P_R"); return GCAMB_EINVAL; }
+    gcamb_los_plan *p = plan;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t nS = (size_t)p->n_k * p->n_tau, nD = (size_t)p->n_src * p->n_l * p->n_k;
+    const size_t nC = (size_t)p->n_spec * p->n_l;
+    if (n_batch > p->host_batch_cap) {
+        for (int q = 0; q < 3; ++q) { cudaFree(p->d_hS[q]); p->d_hS[q] = nullptr; }
+        cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
+        p->d_hP = p->d_hDelta = p->d_hCl = nullptr;
+        p->host_batch_cap = 0;
+        for (int q = 0; q < p->n_src; ++q) GCAMB_CUDA(cudaMalloc(&p->d_hS[q], sizeof(double) * nS * n_batch));
+        GCAMB_CUDA(cudaMalloc(&p->d_hP, sizeof(double) * p->n_k * n_batch));
+        GCAMB_CUDA(cudaMalloc(&p->d_hDelta, sizeof(double) * nD * n_batch));
+        GCAMB_CUDA(cudaMalloc(&p->d_hCl, sizeof(double) * nC * n_batch));
+        p->host_batch_cap = n_batch;
+    }
+    const double *hS[3] = {h_S_T, h_S_E, h_S_phi};
+    for (int q = 0; q < p->n_src; ++q)
+        GCAMB_CUDA(cudaMemcpyAsync(p->d_hS[q], hS[q], sizeof(double) * nS * n_batch, cudaMemcpyHostToDevice, s));
+    GCAMB_CUDA(cudaMemcpyAsync(p->d_hP, h_P_R, sizeof(double) * p->n_k * n_batch, cudaMemcpyHostToDevice, s));
+    st = launch_transfer(p, n_batch, p->d_hS[0], p->d_hS[1], p->d_hS[2], p->d_hDelta, s);
+    if (st != GCAMB_OK) return st;
+    st = launch_cls(p, n_batch, p->d_hDelta, p->d_hP, p->d_hCl, s);
+    if (st != GCAMB_OK) return st;
+    GCAMB_CUDA(cudaMemcpyAsync(h_Cl, p->d_hCl, sizeof(double) * nC * n_batch, cudaMemcpyDeviceToHost, s));
+    if (h_Delta)
+        GCAMB_CUDA(cudaMemcpyAsync(h_Delta, p->d_hDelta, sizeof(double) * nD * n_batch, cudaMemcpyDeviceToHost, s));
+    GCAMB_CUDA(cudaStreamSynchronize(s));
+    return GCAMB_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ DFMA roofline probe
+namespace gcamb {
+__global__ void dfma_probe_kernel(long long iters, double *out)
+{
+    double a[8], m = 1.0 - 1e-9 * (threadIdx.x & 7), c = 1e-12;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) a[q] = 1.0 + q;
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) a[q] = fma(a[q], m, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += a[q];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace gcamb
+
+extern "C" gcamb_status gcamb_los_dfma_probe(int32_t blocks, int32_t threads, int64_t iters, double *d_out,
+                                             void *cuda_stream)
+{
+    if (blocks < 1 || threads < 1 || threads > 1024 || iters < 1 || !d_out) { set_error("bad probe arguments"); return GCAMB_EINVAL; }
+    gcamb::dfma_probe_kernel<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>((long long)iters, d_out);
+    GCAMB_CUDA(cudaGetLastError());
+    return GCAMB_OK;
+}

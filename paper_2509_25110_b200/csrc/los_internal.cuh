@@ -1,0 +1,71 @@
+// Internal declarations shared by the translation units of libgcamb_los.so.
+// Nothing here is visible through the C ABI (include/gcamb_los.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gcamb_los.h"
+
+namespace gcamb {
+
+// Geometry of the transfer kernel chosen at plan creation.
+struct TransferShape {
+    int V;        // l-tile: accumulators per source per thread, = granularity of start tiles
+    int T;        // (k, tau) points ("slots") carried per thread
+    int threads;  // CTA size (multiple of 32)
+    int n_split;  // CTAs sharing one k along tau (1 = plain stores, >1 = fp64 RED into zeroed Delta)
+};
+
+}  // namespace gcamb
+
+struct gcamb_los_plan {
+    int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
+    uint32_t src_mask;
+    double tau0;
+    gcamb::TransferShape shape;
+    int64_t executed_terms;  // sum over (k,tau) of #l in [l_min, min(L(x), l_max)]
+    int64_t walked_terms;    // same with the tile-aligned start the kernel really walks
+    int device;
+
+    // device tables
+    int32_t *d_l_index;  // [l_max+1] position in l_list, or -1
+    double *d_k;         // [n_k]
+    double *d_chi;       // [n_tau] tau0 - tau_i
+    double *d_w;         // [n_tau] trapezoid weights
+    double *d_dlnk;      // [n_k]   trapezoid weights of ln k
+    double *d_pref;      // [n_l]   sqrt((l+2)(l+1)l(l-1))
+    double2 *d_start;    // [n_k][n_tau] (j_{lhi+1}(x), j_{lhi}(x)), lhi = l_max - V*tile
+    int32_t *d_tile;     // [n_k][n_tau] first l-tile of the point
+    int32_t *d_korder;   // [n_k] k indices, heaviest first
+
+    // scratch of gcamb_los_spectra_host (lazily allocated)
+    int32_t host_batch_cap;
+    double *d_hS[3], *d_hP, *d_hDelta, *d_hCl;
+};
+
+namespace gcamb {
+
+void set_error(const char *fmt, ...);
+gcamb_status cuda_fail(cudaError_t e, const char *what);
+
+#define GCAMB_CUDA(call)                                                   \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) return ::gcamb::cuda_fail(e__, #call);     \
+    } while (0)
+
+// plan.cu: fills d_start / d_tile / d_korder / executed_terms on `stream` (synchronises it).
+gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream);
+
+// transfer.cu
+TransferShape choose_shape(int n_tau, int n_src);
+gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                             const double *S_E, const double *S_phi, double *Delta,
+                             cudaStream_t stream);
+
+// cls.cu
+gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,
+                        const double *P_R, double *Cl, cudaStream_t stream);
+
+}  // namespace gcamb

@@ -1,0 +1,153 @@
+// plan.cu -- device-side precompute of a plan: per-(k,tau) recurrence start values.
+//
+// For every point x = k (tau0 - tau) the transfer kernel walks l DOWNWARD from the top of the
+// first l-tile that is not negligible.  This file computes, once per grid set, that tile index
+// and the normalised pair (j_{lhi+1}(x), j_{lhi}(x)) at its top:
+//   * cut (R16):   L(x) = ceil(x + 18.2 x^(1/3) + 8);  |j_l(x)| < 1e-36 for l >= L(x)
+//   * tiles are anchored at l_max: tile t covers l = l_max - V t ... l_max - V t - V + 1
+//   * Miller's backward recurrence (BJ (b)) from M = max(L, lhi) + 50 down to l = 0,
+//     f_{l-1} = (2l+1)/x f_l - f_{l+1}, with power-of-two rescaling against overflow,
+//   * normalised against the closed forms j_0 = sin x / x and j_1 = (sin x / x - cos x)/x with the
+//     two-term least-squares scale of R15 (safe at the zeros of j_0); j_1 by its power series
+//     for x < 1 where the closed form cancels.
+// For x >= l_max the start is in the oscillatory region, where the downward recurrence is
+// neutrally stable (error ~ eps x relative to the envelope, like the forward one).
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+#include <vector>
+
+#include "los_internal.cuh"
+
+namespace gcamb {
+
+__device__ __forceinline__ int l_cut(double x) { return (int)ceil(x + 18.2 * cbrt(x) + 8.0); }
+
+__device__ __forceinline__ double j1_series(double x)
+{
+    // j_1(x) = x/3 (1 - x^2/10 (1 - x^2/28 (1 - x^2/54 ( ... ))));  ratio -x^2 / (2m(2m+3))
+    const double x2 = x * x;
+    double term = x / 3.0, sum = term;
+    for (int m = 1; m < 30; ++m) {
+        term *= -x2 / (double)(2 * m * (2 * m + 3));
+        sum += term;
+        if (fabs(term) < 1e-18 * fabs(sum)) break;
+    }
+    return sum;
+}
+
+__global__ void __launch_bounds__(128) start_values_kernel(const double *__restrict__ k,
+                                                           const double *__restrict__ chi, int n_tau,
+                                                           int l_max, int V,
+                                                           double2 *__restrict__ start,
+                                                           int32_t *__restrict__ tile)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (i >= n_tau) return;
+    const double x = __dmul_rn(k[j], chi[i]);
+    const int L = l_cut(x);
+    const int Ls = min(L, l_max);
+    const int t = (l_max - Ls) / V;
+    const int lhi = l_max - t * V;  // Ls <= lhi < Ls + V
+    const int M = max(L, lhi) + 50;
+
+    double fa = 0.0, fb = 1.0;  // f_{l+1}, f_l
+    double rhi = 0.0, rlo = 0.0;
+    int e = 0, re = 0;
+    for (int l = M; l >= 1; --l) {
+        if (l == lhi) { rlo = fb; rhi = fa; re = e; }
+        const double c = (double)(2 * l + 1) / x;
+        const double fn = fma(c, fb, -fa);
+        fa = fb;
+        fb = fn;
+        if (fabs(fb) > 0x1p500) { fa *= 0x1p-500; fb *= 0x1p-500; ++e; }
+    }
+    // fb = f_0, fa = f_1 (epoch e)
+    double s, c;
+    sincos(x, &s, &c);
+    const double inv = 1.0 / x;
+    const double j0 = s * inv;
+    const double j1 = x < 1.0 ? j1_series(x) : (s * inv - c) * inv;
+    const double m = fmax(fabs(fb), fabs(fa));
+    const double a = fb / m, b = fa / m;
+    const double sc = (j0 * a + j1 * b) / ((a * a + b * b) * m);
+    int e_sc, e_lo, e_hi;
+    const double m_sc = frexp(sc, &e_sc);
+    const double m_lo = frexp(rlo, &e_lo);
+    const double m_hi = frexp(rhi, &e_hi);
+    const int shift = e_sc - 500 * (e - re);
+    double2 out;
+    out.x = ldexp(m_hi * m_sc, e_hi + shift);
+    out.y = ldexp(m_lo * m_sc, e_lo + shift);
+    const size_t idx = (size_t)j * n_tau + i;
+    start[idx] = out;
+    tile[idx] = t;
+}
+
+// per-k work: walked = sum_i (lhi_i - l_min + 1)+, executed = sum_i (min(L(x_i), l_max) - l_min + 1)+
+__global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ k,
+                                                     const double *__restrict__ chi, int n_tau,
+                                                     int l_min, int l_max, int V,
+                                                     const int32_t *__restrict__ tile,
+                                                     long long *__restrict__ walked,
+                                                     long long *__restrict__ executed)
+{
+    __shared__ long long sw[256], se[256];
+    const int j = blockIdx.x;
+    long long w = 0, ex = 0;
+    for (int i = threadIdx.x; i < n_tau; i += blockDim.x) {
+        const double x = __dmul_rn(k[j], chi[i]);
+        const int Ls = min(l_cut(x), l_max);
+        const int lhi = l_max - tile[(size_t)j * n_tau + i] * V;
+        w += max(0, lhi - l_min + 1);
+        ex += max(0, Ls - l_min + 1);
+    }
+    sw[threadIdx.x] = w;
+    se[threadIdx.x] = ex;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s) {
+            sw[threadIdx.x] += sw[threadIdx.x + s];
+            se[threadIdx.x] += se[threadIdx.x + s];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { walked[j] = sw[0]; executed[j] = se[0]; }
+}
+
+gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
+{
+    const int V = p->shape.V;
+    dim3 grid((p->n_tau + 127) / 128, p->n_k);
+    start_values_kernel<<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V,
+                                                  p->d_start, p->d_tile);
+    GCAMB_CUDA(cudaGetLastError());
+
+    long long *d_cost = nullptr;
+    GCAMB_CUDA(cudaMalloc(&d_cost, sizeof(long long) * 2 * (size_t)p->n_k));
+    k_cost_kernel<<<p->n_k, 256, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_min, p->l_max, V,
+                                              p->d_tile, d_cost, d_cost + p->n_k);
+    cudaError_t e = cudaGetLastError();
+    std::vector<long long> cost(2 * (size_t)p->n_k);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(cost.data(), d_cost, sizeof(long long) * cost.size(),
+                            cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    cudaFree(d_cost);
+    if (e != cudaSuccess) return cuda_fail(e, "plan precompute");
+
+    p->walked_terms = std::accumulate(cost.begin(), cost.begin() + p->n_k, 0LL);
+    p->executed_terms = std::accumulate(cost.begin() + p->n_k, cost.end(), 0LL);
+    // heaviest k first: the CTA scheduler hands out blockIdx in order (longest-processing-time rule)
+    std::vector<int32_t> order(p->n_k);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(),
+                     [&](int32_t a, int32_t b) { return cost[a] > cost[b]; });
+    GCAMB_CUDA(cudaMemcpyAsync(p->d_korder, order.data(), sizeof(int32_t) * p->n_k,
+                               cudaMemcpyHostToDevice, stream));
+    GCAMB_CUDA(cudaStreamSynchronize(stream));
+    return GCAMB_OK;
+}
+
+}  // namespace gcamb

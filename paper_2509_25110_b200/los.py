@@ -1,0 +1,179 @@
+"""Thin ctypes binding of libgcamb_los.so (include/gcamb_los.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for device
+memory and streams.  There is no CPU fallback: if the library is missing or no CUDA device is
+present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgcamb_los.so")
+
+GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI = 1, 2, 4
+_STATUS = {0: "GCAMB_OK", 1: "GCAMB_EINVAL", 2: "GCAMB_EGRID", 3: "GCAMB_EALLOC", 4: "GCAMB_ECUDA"}
+
+EXPORTS = (
+    "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_transfer",
+    "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
+    "gcamb_los_dfma_probe", "gcamb_los_last_error",
+)
+
+_vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+_lib = None
+
+
+class GcambError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree library; fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2509_25110_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.gcamb_los_last_error.restype = ctypes.c_char_p
+    lib.gcamb_los_plan_create.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64,
+                                          ctypes.c_uint32, _vp]
+    lib.gcamb_los_plan_destroy.argtypes = [_vp]
+    lib.gcamb_los_plan_info.argtypes = [_vp] + [ctypes.POINTER(_i32)] * 5 + [ctypes.POINTER(_i64)]
+    lib.gcamb_los_transfer.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_cls.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_transfer_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_cls_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_spectra_host.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_dfma_probe.argtypes = [_i32, _i32, _i64, _vp, _vp]
+    _lib = lib
+    return lib
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise GcambError(status, load_library().gcamb_los_last_error().decode())
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dev(t: torch.Tensor | None, shape, name: str) -> int | None:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name}: need a contiguous float64 CUDA tensor")
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return t.data_ptr()
+
+
+def _host(a, shape, name: str) -> np.ndarray | None:
+    if a is None:
+        return None
+    if isinstance(a, torch.Tensor):
+        a = a.numpy()
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous):
+        raise TypeError(f"{name}: need a C-contiguous float64 host array")
+    if tuple(a.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(a.shape)} != {tuple(shape)}")
+    return a
+
+
+class Plan:
+    """gcamb_los_plan: grids, quadrature weights and recurrence start values on the device."""
+
+    def __init__(self, l_list, k, tau, tau0: float, with_phi: bool = False):
+        if not torch.cuda.is_available():
+            raise RuntimeError("gcamb_los needs a CUDA device (no CPU fallback)")
+        lib = load_library()
+        l_list = np.ascontiguousarray(l_list, dtype=np.int32)
+        k = np.ascontiguousarray(k, dtype=np.float64)
+        tau = np.ascontiguousarray(tau, dtype=np.float64)
+        mask = GCAMB_SRC_T | GCAMB_SRC_E | (GCAMB_SRC_PHI if with_phi else 0)
+        handle = _vp()
+        _check(lib.gcamb_los_plan_create(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
+                                         k.ctypes.data, k.size, tau.ctypes.data, tau.size,
+                                         float(tau0), mask, _stream()))
+        self._h = handle
+        out = [_i32() for _ in range(5)]
+        ex = _i64()
+        _check(lib.gcamb_los_plan_info(self._h, *[ctypes.byref(o) for o in out], ctypes.byref(ex)))
+        self.n_l, self.n_k, self.n_tau, self.n_src, self.n_spec = (o.value for o in out)
+        self.executed_terms = ex.value
+        self.nominal_terms = self.n_l * self.n_k * self.n_tau
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            _check(load_library().gcamb_los_plan_destroy(self._h))
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- device-resident calls (asynchronous on torch's current stream)
+    def gcamb_los_transfer(self, S_T, S_E, S_phi=None, out=None) -> torch.Tensor:
+        return self.gcamb_los_transfer_batched(S_T, S_E, S_phi, out, _batched=False)
+
+    def gcamb_los_transfer_batched(self, S_T, S_E, S_phi=None, out=None, _batched=True) -> torch.Tensor:
+        B = (S_T.shape[0],) if _batched else ()
+        sh = B + (self.n_k, self.n_tau)
+        if out is None:
+            out = torch.empty(B + (self.n_src, self.n_l, self.n_k), dtype=torch.float64, device=S_T.device)
+        pT, pE, pP = _dev(S_T, sh, "S_T"), _dev(S_E, sh, "S_E"), _dev(S_phi, sh, "S_phi")
+        pD = _dev(out, B + (self.n_src, self.n_l, self.n_k), "Delta")
+        lib = load_library()
+        if _batched:
+            _check(lib.gcamb_los_transfer_batched(self._h, B[0], pT, pE, pP, pD, _stream()))
+        else:
+            _check(lib.gcamb_los_transfer(self._h, pT, pE, pP, pD, _stream()))
+        return out
+
+    def gcamb_los_cls(self, Delta, P_R, out=None) -> torch.Tensor:
+        return self.gcamb_los_cls_batched(Delta, P_R, out, _batched=False)
+
+    def gcamb_los_cls_batched(self, Delta, P_R, out=None, _batched=True) -> torch.Tensor:
+        B = (Delta.shape[0],) if _batched else ()
+        if out is None:
+            out = torch.empty(B + (self.n_spec, self.n_l), dtype=torch.float64, device=Delta.device)
+        pD = _dev(Delta, B + (self.n_src, self.n_l, self.n_k), "Delta")
+        pP = _dev(P_R, B + (self.n_k,), "P_R")
+        pC = _dev(out, B + (self.n_spec, self.n_l), "Cl")
+        lib = load_library()
+        if _batched:
+            _check(lib.gcamb_los_cls_batched(self._h, B[0], pD, pP, pC, _stream()))
+        else:
+            _check(lib.gcamb_los_cls(self._h, pD, pP, pC, _stream()))
+        return out
+
+    # ---- host buffers in, host buffers out (H2D + kernels + D2H inside the call)
+    def gcamb_los_spectra_host(self, S_T, S_E, S_phi, P_R, Cl_out, Delta_out=None) -> None:
+        B = S_T.shape[0]
+        sh = (B, self.n_k, self.n_tau)
+        aT, aE, aP = _host(S_T, sh, "S_T"), _host(S_E, sh, "S_E"), _host(S_phi, sh, "S_phi")
+        aR = _host(P_R, (B, self.n_k), "P_R")
+        aC = _host(Cl_out, (B, self.n_spec, self.n_l), "Cl")
+        aD = _host(Delta_out, (B, self.n_src, self.n_l, self.n_k), "Delta")
+        _check(load_library().gcamb_los_spectra_host(
+            self._h, B, aT.ctypes.data, aE.ctypes.data, None if aP is None else aP.ctypes.data,
+            aR.ctypes.data, aC.ctypes.data, None if aD is None else aD.ctypes.data, _stream()))
+
+
+def gcamb_los_plan_create(l_list, k, tau, tau0, with_phi=False) -> Plan:
+    return Plan(l_list, k, tau, tau0, with_phi)
+
+
+def gcamb_los_dfma_probe(blocks: int, threads: int, iters: int, out: torch.Tensor) -> None:
+    _check(load_library().gcamb_los_dfma_probe(blocks, threads, iters, _dev(out, (blocks * threads,), "out"), _stream()))

@@ -1,0 +1,170 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):  |Delta_GPU - Delta_oracle| <= 1e-10 * max_k |Delta_l|  per l and
+source;  C_l relative error <= 1e-8 for TT, EE, phiphi; for TE, which crosses zero, the same bound
+relative to sqrt(C_TE^2 + C_TT C_EE) (reading R13, the paper's own TE normaliser, Eq. 5
+PAPER.md:237).  The grading oracle is the long-double build (R14); the fp64 build is checked too.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2509_25110_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_DELTA = 1e-10
+TOL_CL = 1e-8
+
+
+@pytest.fixture(scope="module")
+def los():
+    from paper_2509_25110_b200 import los as _los
+    _los.load_library()
+    assert torch.cuda.is_available()
+    return _los
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def delta_err(D_gpu, D_ref, scale=None):
+    """max over (source, l) of max_k |diff| / max_k |Delta_l|."""
+    if scale is None:
+        scale = np.max(np.abs(D_ref), axis=-1, keepdims=True)
+    scale = np.where(scale > 0, scale, 1.0)
+    return float(np.max(np.abs(D_gpu - D_ref) / scale))
+
+
+def cl_err(C_gpu, C_ref):
+    auto = [0, 1] + ([3] if C_ref.shape[-2] == 4 else [])
+    e_auto = float(np.max(np.abs(C_gpu[..., auto, :] / C_ref[..., auto, :] - 1.0)))
+    norm = np.sqrt(C_ref[..., 2, :] ** 2 + C_ref[..., 0, :] * C_ref[..., 1, :])
+    e_te = float(np.max(np.abs(C_gpu[..., 2, :] - C_ref[..., 2, :]) / norm))
+    return e_auto, e_te
+
+
+def run_gpu(los, l_list, k, tau, tau0, S_T, S_E, S_P, P_R):
+    plan = los.Plan(l_list, k, tau, tau0, with_phi=S_P is not None)
+    D = plan.gcamb_los_transfer(dev(S_T), dev(S_E), None if S_P is None else dev(S_P))
+    C = plan.gcamb_los_cls(D, dev(P_R))
+    torch.cuda.synchronize()
+    out = D.cpu().numpy(), C.cpu().numpy(), plan
+    return out
+
+
+# --------------------------------------------------------------------------- config 0, element by element
+@pytest.mark.parametrize("real", ["f80", "f64"])
+def test_config0_full_parity(los, real):
+    cfg = synth.CONFIGS[0]
+    S_T, S_E, _ = synth.sources(cfg)
+    P = synth.primordial_power(cfg)
+    D, C, plan = run_gpu(los, cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, S_T, S_E, None, P)
+    assert plan.nominal_terms == cfg.nominal_terms()
+    assert 0 < plan.executed_terms < plan.nominal_terms
+    D_ref = oracle.transfer(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, S_T, S_E, real=real)
+    C_ref = oracle.cls(cfg.k(), D_ref, P, real=real)
+    assert delta_err(D, D_ref) <= TOL_DELTA
+    e_auto, e_te = cl_err(C, C_ref)
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+    # the C_l kernel alone, fed the oracle's Delta
+    C2 = plan.gcamb_los_cls(dev(D_ref), dev(P)).cpu().numpy()
+    e_auto, e_te = cl_err(C2, C_ref)
+    assert e_auto <= 1e-13 and e_te <= 1e-13
+
+
+# --------------------------------------------------------------------------- ragged / edge shapes
+def _small_problem(n_l_spec, n_k, n_tau, with_phi, seed):
+    rng = np.random.default_rng(seed)
+    tau0 = 14000.0
+    tau = np.sort(rng.uniform(50.0, 13990.0, n_tau))
+    tau[-1] = 13999.5
+    k = np.geomspace(3e-5, 0.11, n_k) * (1 + 0.01 * rng.uniform(-1, 1, n_k))
+    k.sort()
+    S = [rng.standard_normal((n_k, n_tau)) for _ in range(3)]
+    P = rng.uniform(1e-9, 3e-9, n_k)
+    return n_l_spec, k, tau, tau0, S[0], S[1], S[2] if with_phi else None, P
+
+
+@pytest.mark.parametrize("case", [
+    (np.arange(2, 200), 33, 97, False, 1),            # ragged tau (not a multiple of 32 or of the CTA)
+    (np.arange(2, 77), 5, 2, True, 2),                # minimum n_tau
+    (np.array([2]), 2, 40, False, 3),                 # single l, minimum n_k
+    (np.array([5, 6, 40, 41, 300, 1500]), 17, 300, True, 4),    # sparse l list (R21), x up to 1540
+    (np.arange(700, 900), 9, 130, False, 5),          # l range not starting at 2
+    (np.arange(2, 40), 12, 1300, True, 6),            # n_tau above one CTA's slots for n_src=3
+    (np.arange(2, 60), 6, 3100, False, 7),            # tau split across CTAs (RED path), n_src=2
+])
+def test_edge_shapes(los, case):
+    l_list, k, tau, tau0, S_T, S_E, S_P, P = _small_problem(*case)
+    l_list = np.asarray(l_list, dtype=np.int32)
+    D, C, _ = run_gpu(los, l_list, k, tau, tau0, S_T, S_E, S_P, P)
+    D_ref = oracle.transfer(l_list, k, tau, tau0, S_T, S_E, S_P, real="f80")
+    C_ref = oracle.cls(k, D_ref, P, real="f80")
+    assert D.shape == D_ref.shape and C.shape == C_ref.shape
+    assert delta_err(D, D_ref) <= TOL_DELTA
+    e_auto, e_te = cl_err(C, C_ref)
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+
+
+def test_single_tau_source_is_the_kernel(los):
+    """P3 on the GPU: S = delta_{i,i*}/w_{i*} gives Delta_l(k) = j_l(k chi*) (values: oracle column)."""
+    tau = np.array([100.0, 280.0, 700.0, 13000.0])
+    k = np.geomspace(2e-4, 0.2, 50)
+    S = np.zeros((k.size, tau.size)); S[:, 1] = 1.0 / 300.0
+    l_list = np.arange(2, 1200, dtype=np.int32)
+    D, _, _ = run_gpu(los, l_list, k, tau, 14000.0, S, S, S, np.ones(k.size))
+    for j in (0, 13, 37, 49):
+        x = float(k[j] * (14000.0 - 280.0))
+        jl = oracle.sph_bessel(x, 1199, real="f80")[2:]
+        assert np.max(np.abs(D[0, :, j] - jl)) <= 3e-12 / max(x, 1.0) + 1e-300
+        assert np.array_equal(D[2, :, j], D[0, :, j])
+
+
+# --------------------------------------------------------------------------- batched == loop of single
+def test_batched_equals_loop_of_single(los):
+    cfg = synth.Config(9, "mini-batch", 2, 300, 64, 1e-4, 0.25, 120, 60, False, n_batch=5)
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0)
+    S = [synth.sources(cfg, c) for c in range(cfg.n_batch)]
+    S_T = dev(np.stack([s[0] for s in S])); S_E = dev(np.stack([s[1] for s in S]))
+    P = dev(np.stack([synth.primordial_power(cfg, c) for c in range(cfg.n_batch)]))
+    Db = plan.gcamb_los_transfer_batched(S_T, S_E)
+    Cb = plan.gcamb_los_cls_batched(Db, P)
+    for c in range(cfg.n_batch):
+        D1 = plan.gcamb_los_transfer(S_T[c].contiguous(), S_E[c].contiguous())
+        C1 = plan.gcamb_los_cls(D1, P[c].contiguous())
+        assert torch.equal(D1, Db[c]) and torch.equal(C1, Cb[c])     # bit-exact: same kernels, same order
+    D_ref = oracle.transfer(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, S[3][0], S[3][1], real="f80")
+    assert delta_err(Db[3].cpu().numpy(), D_ref) <= TOL_DELTA
+
+
+def test_host_buffer_entry_point_matches_device_path(los):
+    cfg = synth.Config(9, "mini", 2, 150, 48, 1e-4, 0.2, 100, 50, True)
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, with_phi=True)
+    S_T, S_E, S_P = synth.sources(cfg)
+    P = synth.primordial_power(cfg)
+    D = plan.gcamb_los_transfer(dev(S_T), dev(S_E), dev(S_P))
+    C = plan.gcamb_los_cls(D, dev(P))
+    Cl = np.empty((1, 4, cfg.n_l)); Dl = np.empty((1, 3, cfg.n_l, cfg.n_k))
+    plan.gcamb_los_spectra_host(S_T[None], S_E[None], S_P[None], P[None], Cl, Dl)
+    assert np.array_equal(Cl[0], C.cpu().numpy()) and np.array_equal(Dl[0], D.cpu().numpy())
+
+
+def test_errors_cross_the_abi_as_status_codes(los):
+    cfg = synth.CONFIGS[0]
+    with pytest.raises(los.GcambError) as e:
+        los.Plan(cfg.l_list(), cfg.k()[::-1].copy(), cfg.tau(), cfg.tau0)
+    assert e.value.status == 2
+    with pytest.raises(los.GcambError) as e:
+        los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau()[-1])       # x = 0 (R18)
+    assert e.value.status == 2
+    with pytest.raises(los.GcambError) as e:
+        los.Plan([1, 2, 3], cfg.k(), cfg.tau(), cfg.tau0)
+    assert e.value.status == 1
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0)
+    z = torch.zeros(cfg.n_k, cfg.n_tau, dtype=torch.float64, device="cuda")
+    with pytest.raises(los.GcambError) as e:
+        plan.gcamb_los_transfer(z, z, z)                                # phi source without the mask bit
+    assert e.value.status == 1
