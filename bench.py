@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the line-of-sight hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+A step = one pass of the whole hot path, gcamb_los_transfer + gcamb_los_cls (their batched
+forms at config 3), over one batch of seeded synthetic sources that is already resident in HBM.
+Default workload: BASELINE.json config 1 ("CAMB-default-scale", l = 2..2500), the config the
+metric is quoted on.  `value` = nominal (l,k,tau) terms per second = N_l N_k N_tau B per step /
+device time per step (reading R19); the executed-term rate (terms not skipped by R16), spectra/s
+and the FP64 roofline of the transfer kernel are reported beside it.
+
+N > 1 (torchrun): every rank runs its own cosmology of the same grid (independent problems, no
+data-path collective: DESIGN.md "Multi-GPU"), `value` = all ranks' terms / max-over-ranks time.
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores on a
+bounded k-sample of the same workload; there is no reference implementation to install.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2509_25110_b200 import synth  # noqa: E402  (generator only: none of the method's arithmetic)
+
+METRIC = "LOS (l,k,tau) terms/s at lmax=2500"
+UNIT = "terms/s"
+# FP64 roofline denominator: 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz
+FP64_LANES_PER_SM = 64
+L2_FLUSH_BYTES = 256 << 20
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:  # pragma: no cover
+        return os.cpu_count() or 1
+
+
+def workload_config(cfg) -> dict:
+    return {
+        "workload": f"config {cfg.index} ({cfg.name}): l={cfg.l_min}..{cfg.l_max} (all), n_k={cfg.n_k} log in "
+                    f"[{cfg.k_lo:g},{cfg.k_hi:g}], n_tau={cfg.n_tau} ({cfg.n_tau_uniform} uniform + "
+                    f"{cfg.n_tau_log} log), sources T,E{',phi' if cfg.with_phi else ''}, batch={cfg.n_batch}",
+        "n_l": cfg.n_l, "n_k": cfg.n_k, "n_tau": cfg.n_tau, "n_src": cfg.n_src, "batch": cfg.n_batch,
+        "seed": cfg.seed,
+    }
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and clock-event reasons through NVML (what nvidia-smi reads) in a thread."""
+
+    REASONS = {
+        0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+        0x4: "sw_power_cap", 0x80: "hw_power_brake", 0x2: "applications_clocks_setting",
+        0x100: "display_clock_setting", 0x10: "sync_boost",
+    }
+
+    def __init__(self, torch_device_index: int, period_s: float = 0.02):
+        self.period = period_s
+        self.samples: list[int] = []
+        self.reason_bits = 0
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            uuid = getattr(torch.cuda.get_device_properties(torch_device_index), "uuid", None)
+            try:
+                self._h = pynvml.nvmlDeviceGetHandleByUUID(f"GPU-{uuid}".encode())
+            except Exception:
+                self._h = pynvml.nvmlDeviceGetHandleByIndex(torch_device_index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # NVML missing: report that instead of inventing clocks
+            self.error = repr(e)
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    bits = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                except Exception:
+                    bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                self.reason_bits |= int(bits)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self._h is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0,
+                    "error": getattr(self, "error", "no samples")}
+        reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit]
+        return {"sm_mhz": float(np.median(self.samples)), "sm_min_mhz": int(min(self.samples)),
+                "sm_max_mhz": self.sm_max, "reasons": reasons, "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------- reference arm
+def oracle_sample_run(cfg, stride: int, cores: int):
+    """The oracle as it stands (fp64 build, OpenMP over k) on every `stride`-th k row of the workload."""
+    import oracle
+    sl = slice(0, cfg.n_k, stride)
+    sl_k = cfg.k()[sl]
+    S_T, S_E, S_P = synth.sources(cfg, 0, sl)
+    P = synth.primordial_power(cfg, 0)[sl]
+    t0 = time.perf_counter()
+    D = oracle.transfer(cfg.l_list(), sl_k, cfg.tau(), cfg.tau0, S_T, S_E, S_P, real="f64", nthreads=cores)
+    C = oracle.cls(sl_k, D, P, real="f64", nthreads=cores)
+    dt = time.perf_counter() - t0
+    return dt, D, C, np.arange(cfg.n_k)[sl]
+
+
+def calibrate_stride(cfg, cores: int, budget_s: float) -> int:
+    """k stride whose sample costs about `budget_s` of oracle time (every cost class of the
+    ragged workload stays represented: the rows are evenly strided over the log-spaced k grid)."""
+    probe = max(1, cfg.n_k // max(2 * cores, 16))
+    dt, _, _, rows = oracle_sample_run(cfg, probe, cores)
+    per_row = dt / rows.size
+    n_rows = max(2, min(cfg.n_k, int(budget_s / max(per_row, 1e-9))))
+    return max(1, -(-cfg.n_k // n_rows))
+
+
+def run_reference(args) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    cfg = synth.CONFIGS[args.config]
+    cores = host_cores()
+    budget = min(20.0, 150.0 / max(1, args.steps + args.warmup))
+    stride = calibrate_stride(cfg, cores, budget)
+    for _ in range(args.warmup):
+        oracle_sample_run(cfg, stride, cores)
+    runs = [oracle_sample_run(cfg, stride, cores) for _ in range(args.steps)]
+    t = float(np.mean([r[0] for r in runs]))
+    n_rows = runs[0][3].size
+    terms = cfg.n_l * n_rows * cfg.n_tau
+    value = terms / t
+    sample = f"every {stride}-th k row ({n_rows} of {cfg.n_k}), all l, all tau, one cosmology per step"
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+# --------------------------------------------------------------------------- CUDA arm
+def run_cuda(args) -> None:
+    import torch
+
+    from paper_2509_25110_b200 import los
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    los.load_library()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = synth.CONFIGS[args.config]
+    B = cfg.n_batch
+    batched = B > 1
+    props = torch.cuda.get_device_properties(dev)
+    n_sm = props.multi_processor_count
+
+    # ---- inputs: pinned host copies (for the e2e leg) and device-resident copies (for `value`)
+    first_c = rank * B
+    hS = [[], [], []]
+    for c in range(first_c, first_c + B):
+        s = synth.sources(cfg, c)
+        for q in range(cfg.n_src):
+            hS[q].append(s[q])
+    hS = [torch.from_numpy(np.stack(x)).pin_memory() if x else None for x in hS]
+    hP = torch.from_numpy(np.stack([synth.primordial_power(cfg, c) for c in range(first_c, first_c + B)])).pin_memory()
+    dS = [None if x is None else (x.to(dev) if batched else x[0].to(dev)) for x in hS]
+    dP = hP.to(dev) if batched else hP[0].to(dev)
+
+    t0 = time.perf_counter()
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, with_phi=cfg.with_phi)
+    torch.cuda.synchronize()
+    plan_ms = 1e3 * (time.perf_counter() - t0)
+
+    lead = (B,) if batched else ()
+    Delta = torch.empty(lead + (plan.n_src, plan.n_l, plan.n_k), dtype=torch.float64, device=dev)
+    Cl = torch.empty(lead + (plan.n_spec, plan.n_l), dtype=torch.float64, device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    def transfer():
+        if batched:
+            plan.gcamb_los_transfer_batched(dS[0], dS[1], dS[2], out=Delta)
+        else:
+            plan.gcamb_los_transfer(dS[0], dS[1], dS[2], out=Delta)
+
+    def cls():
+        if batched:
+            plan.gcamb_los_cls_batched(Delta, dP, out=Cl)
+        else:
+            plan.gcamb_los_cls(Delta, dP, out=Cl)
+
+    launches_per_step = plan.launches_per_step
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        transfer()
+        cls()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    wall0 = time.perf_counter()
+    for s in range(args.steps):
+        flush.zero_()                      # > L2 (126 MB): every step starts with a cold L2
+        ev[s][0].record()
+        transfer()
+        ev[s][1].record()
+        cls()
+        ev[s][2].record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    t_transfer = np.array([e[0].elapsed_time(e[1]) for e in ev]) * 1e-3
+    t_cls = np.array([e[1].elapsed_time(e[2]) for e in ev]) * 1e-3
+    t_step = float(np.mean(t_transfer + t_cls))
+
+    # ---- e2e: the public host-buffer call, H2D of the sources and D2H of C_l inside the timed region
+    hCl = torch.empty((B, plan.n_spec, plan.n_l), dtype=torch.float64).pin_memory()
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(2):
+        plan.gcamb_los_spectra_host(hS[0], hS[1], hS[2], hP, hCl)
+    barrier()
+    e0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.gcamb_los_spectra_host(hS[0], hS[1], hS[2], hP, hCl)   # synchronises its stream
+    torch.cuda.synchronize()
+    t_e2e = (time.perf_counter() - e0) / e2e_steps
+    barrier()
+    same = bool(np.array_equal(hCl.numpy().reshape(Cl.shape), Cl.cpu().numpy()))
+    h2d = sum(int(x.numel()) * 8 for x in hS if x is not None) + int(hP.numel()) * 8
+    d2h = int(hCl.numel()) * 8
+
+    # ---- max over ranks
+    tt = torch.tensor([t_step, t_e2e, float(np.mean(t_transfer)), float(np.mean(t_cls))], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_step, t_e2e, t_tr, t_cl = (float(v) for v in tt.cpu())
+
+    nominal = plan.nominal_terms * B
+    executed = plan.executed_terms * B
+    flop_per_term = 2 * (2 + plan.n_src)             # coefficient + recurrence + n_src accumulate DFMAs
+    peak_tf = n_sm * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    achieved_tf = executed * flop_per_term / t_tr / 1e12
+
+    # measured DFMA ceiling of this device, same process (dependent chains, 8 per thread)
+    probe_out = torch.empty(n_sm * 8 * 256, dtype=torch.float64, device=dev)
+    iters = 1 << 14
+    los.gcamb_los_dfma_probe(n_sm * 8, 256, iters, probe_out)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    los.gcamb_los_dfma_probe(n_sm * 8, 256, iters, probe_out)
+    p1.record()
+    torch.cuda.synchronize()
+    probe_tf = n_sm * 8 * 256 * 8 * iters * 2 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    out = {
+        "metric": METRIC, "value": nominal * world / t_step, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {**workload_config(cfg), "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB memset)",
+                   "per_rank": "one cosmology batch per GPU, no collective on the data path"},
+        "executed_terms_per_s": executed * world / t_step,
+        "executed_fraction": plan.executed_terms / plan.nominal_terms,
+        "spectra_per_s": B * world / t_step,
+        "transfer_ms": 1e3 * t_tr, "cls_ms": 1e3 * t_cl, "plan_create_ms": plan_ms,
+        "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
+        "clocks": clocks,
+        "e2e": {"value": nominal * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e, "api": "gcamb_los_spectra_host",
+                "matches_device_path": same},
+        "gpu_launches": launches_per_step * args.steps,
+        "roofline": {
+            "bound": "alu", "kernel": "transfer_kernel", "achieved": achieved_tf, "peak": peak_tf,
+            "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+            "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
+                           f"dfma probe measured {probe_tf:.2f} TFLOP/s in this process",
+            "algorithmic": f"{flop_per_term} flop per executed term x {executed} executed terms per launch",
+            "frac_of_measured_dfma": achieved_tf / probe_tf,
+        },
+    }
+
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        cores = host_cores()
+        stride = calibrate_stride(cfg, cores, 15.0)
+        dt, D_ref, _, rows = oracle_sample_run(cfg, stride, cores)
+        D_gpu = (Delta[0] if batched else Delta)[:, :, torch.from_numpy(rows).to(dev)].cpu().numpy()
+        scale = np.max(np.abs(D_ref), axis=-1, keepdims=True)
+        err = float(np.max(np.abs(D_gpu - D_ref) / np.where(scale > 0, scale, 1.0)))
+        out["cpu_baseline"] = {
+            "value": cfg.n_l * rows.size * cfg.n_tau / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"every {stride}-th k row ({rows.size} of {cfg.n_k}), all l, all tau, cosmology 0; "
+                      f"fp64 oracle build, {dt:.1f} s",
+            "delta_err_on_sample": err,
+        }
+    print(json.dumps(out), flush=True)
+    plan.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--config", type=int, default=1, choices=range(len(synth.CONFIGS)))
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 3 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        run_reference(args)
+    else:
+        args.steps = 100 if args.steps is None else args.steps
+        args.warmup = 5 if args.warmup is None else max(args.warmup, 3)
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

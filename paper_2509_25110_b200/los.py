@@ -111,6 +111,8 @@ class Plan:
         self.n_l, self.n_k, self.n_tau, self.n_src, self.n_spec = (o.value for o in out)
         self.executed_terms = ex.value
         self.nominal_terms = self.n_l * self.n_k * self.n_tau
+        # kernels of this library one transfer + one cls call launch (bench.py's gpu_launches)
+        self.launches_per_step = 2
 
     def close(self) -> None:
         if getattr(self, "_h", None):
