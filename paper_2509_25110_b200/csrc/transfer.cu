@@ -8,11 +8,18 @@
 //     acc_X[l] += s_X * f_l                 n_src DFMA
 //     f_{l-1} = c * f_l - f_{l+1}           1 DFMA
 // i.e. 2 + n_src FP64 issue slots per executed (l,k,tau) term, no j_l table, no sincos: the start
-// pair of each point comes from the plan (plan.cu).  After a tile the V x n_src per-thread sums
-// are reduced across the warp with a transposing butterfly (1 DADD + 1 double SHFL per l and
-// source), across warps through shared memory, scaled (Delta^E prefactor) and stored.
-// Points whose cut L(x) lies below the current tile are not walked at all (R16): whole slots
-// are skipped with a warp-uniform branch, single lanes are predicated off.
+// pair of each point comes from the plan (plan.cu) and is injected when the walk reaches the
+// point's first tile; until then the point carries f = 0 and contributes exactly 0 (R16).
+//
+// Ragged work: x falls with tau, so within a warp slot j starts no earlier than slot j-1.  The
+// tile body is instantiated for every number NA of started slots (warp-uniform), so slots that
+// have not started cost nothing and started ones always run as NA interleaved chains.
+//
+// Reduction: after a tile the V x n_src per-thread sums are reduced across the warp with a
+// transposing butterfly (1 DADD + 1 double SHFL per l and source) into a shared-memory ring;
+// every G tiles the CTA synchronises once, sums the warps in fixed order, applies the Delta^E
+// prefactor and stores.  The summation order is fixed by the launch shape alone, so results are
+// bit-reproducible and the batched call equals a loop of single calls.
 #include "los_internal.cuh"
 
 namespace gcamb {
@@ -27,6 +34,7 @@ struct TransferParams {
 };
 
 constexpr unsigned FULL = 0xffffffffu;
+constexpr int NEVER = 0x7fffffff;
 
 // a[s] (s < V) per lane  ->  sum over the 32 lanes of a[s], returned on every lane for
 // s = lane / (32 / V).  V/2 + V/4 + ... + 1 exchanges, then log2(32/V) plain butterfly steps.
@@ -49,11 +57,35 @@ __device__ __forceinline__ double warp_transpose_reduce(double (&a)[V], int lane
     return a[0];
 }
 
-template <int T, int V, int NSRC, int MAXTHREADS, int MINBLOCKS>
+// a2 + a3 for one l-tile and the first NA slots of this thread: NA independent recurrence chains.
+template <int NA, int T, int V, int NSRC>
+__device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], const double (&src)[NSRC][T],
+                                          double (&fa)[T], double (&fb)[T], double (&acc)[NSRC][V])
+{
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+        const double tl = tl0 - 2.0 * s;   // 2l+1
+#pragma unroll
+        for (int j = 0; j < NA; ++j) {
+            const double c = tl * ix[j];
+#pragma unroll
+            for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
+            const double fn = fma(c, fb[j], -fa[j]);
+            fa[j] = fb[j];
+            fb[j] = fn;
+        }
+    }
+}
+
+template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
-    extern __shared__ double red[];  // [2][W][NSRC][V]
+    static_assert(T >= 1 && T <= 10, "the NA dispatch below is written out for T <= 10");
+    extern __shared__ double2 smem2[];   // start pairs [T][threads], ring [2][G][W][NSRC][V], slot starts [W][T]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+    double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
+    double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x);
+    int *slot_start = reinterpret_cast<int *>(ring + (size_t)2 * G * W * NSRC * V);
     const int bid = blockIdx.x;
     const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;
     const int kidx = p.korder[krank];
@@ -61,43 +93,43 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const int i_begin = split * p.split_len;
     const int i_end = min(p.n_tau, i_begin + p.split_len);
     const double kval = p.k[kidx];
+    const size_t row = (size_t)kidx * p.n_tau;
 
-    // ---- a1: source staging.  slot j of this thread is tau index i_begin + j*blockDim + tid.
+    // ---- a1: source staging.  Slot j of the CTA covers tau indices i_begin + j*blockDim ...
+    // + blockDim - 1, dealt round-robin to the warps (lane*W + warp) so that every warp sees the
+    // same mix of start tiles and the warps of a CTA stay in step between flushes.
     double fa[T], fb[T], ix[T], src[NSRC][T];
     int tp[T];
-    int tall = -1;   // last start tile among this thread's valid points
-    int nslot = 0;   // slots of this WARP that hold at least one valid point (warp-uniform)
+    const int i_mine = i_begin + lane * W + warp;
 #pragma unroll
     for (int j = 0; j < T; ++j) {
-        const int i = i_begin + j * (int)blockDim.x + tid;
-        if (i - lane < i_end) nslot = j + 1;
+        const int i = i_mine + j * (int)blockDim.x;
+        fa[j] = fb[j] = 0.0;
         if (i < i_end) {
-            const size_t pt = (size_t)kidx * p.n_tau + i;
             const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + i;
             const double x = __dmul_rn(kval, p.chi[i]);
             const double inv = 1.0 / x;
             const double w = p.w[i];
-            const double2 st = p.start[pt];
-            fa[j] = st.x;
-            fb[j] = st.y;
             ix[j] = inv;
-            tp[j] = p.tile[pt];
-            tall = max(tall, tp[j]);
+            tp[j] = p.tile[row + i];
+            my_start[j * blockDim.x] = p.start[row + i];
             src[0][j] = w * p.S[0][sx];
             src[1][j] = w * p.S[1][sx] * (inv * inv);
             if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
         } else {
-            fa[j] = fb[j] = ix[j] = 0.0;
-            tp[j] = 0x7fffffff;
+            ix[j] = 0.0;
+            tp[j] = NEVER;
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) src[q][j] = 0.0;
         }
+        // x falls with tau: the slot starts with its first lane, and slot j never before slot j-1
+        const int first = __reduce_min_sync(FULL, tp[j]);
+        if (lane == 0) slot_start[warp * T + j] = first;
     }
-    tall = __reduce_max_sync(FULL, tall);
-    const bool warp_full = nslot == T;
+    __syncwarp();
 
-    // first tile of this CTA = start tile of its largest x (tau is increasing, x decreasing)
-    const int t_begin = p.tile[(size_t)kidx * p.n_tau + i_begin];
+    // first tile of this CTA = start tile of its largest x
+    const int t_begin = p.tile[row + i_begin];
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
 
     // l above the first tile: Delta is exactly zero there (R16).  With RED output the buffer was
@@ -113,103 +145,135 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         }
     }
 
-    int buf = 0;
+    int na = 0;                               // started slots of this warp (warp-uniform)
+    int next_slot = slot_start[warp * T];     // tile at which slot `na` starts
+    int phase = 0, g = 0, t_flush = t_begin;  // ring bookkeeping (CTA-uniform)
     for (int t = t_begin; t < p.n_tiles; ++t) {
-        const int lhi = p.l_max - t * V;
-        const double tl0 = (double)(2 * lhi + 1);
-        double acc[NSRC][V];
+        while (next_slot <= t) {
+            ++na;
+            next_slot = na < T ? slot_start[warp * T + na] : NEVER;
+        }
+        // inject the plan's start pair (j_{lhi+1}, j_lhi) into points whose walk begins here
 #pragma unroll
-        for (int q = 0; q < NSRC; ++q)
-#pragma unroll
-            for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
+        for (int j = 0; j < T; ++j) {
+            if (tp[j] == t) {
+                const double2 st = my_start[j * blockDim.x];
+                fa[j] = st.x;
+                fb[j] = st.y;
+            }
+        }
 
-        if (warp_full && t >= tall) {
-            // ---- a2 + a3, steady state: every point of the warp is active; T independent chains
+        double *rb = ring + ((size_t)(phase * G + g) * W + warp) * NSRC * V;
+        if (na > 0) {
+            const double tl0 = (double)(2 * (p.l_max - t * V) + 1);
+            double acc[NSRC][V];
 #pragma unroll
-            for (int s = 0; s < V; ++s) {
-                const double tl = tl0 - 2.0 * s;
+            for (int q = 0; q < NSRC; ++q)
 #pragma unroll
-                for (int j = 0; j < T; ++j) {
-                    const double c = tl * ix[j];
+                for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
+#define GCAMB_NA(n) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC>(tl0, ix, src, fa, fb, acc); break;
+            switch (na) {
+                GCAMB_NA(1) GCAMB_NA(2) GCAMB_NA(3) GCAMB_NA(4) GCAMB_NA(5)
+                GCAMB_NA(6) GCAMB_NA(7) GCAMB_NA(8) GCAMB_NA(9) GCAMB_NA(10)
+            }
+#undef GCAMB_NA
+            // cross-lane reduction into this warp's ring entry
 #pragma unroll
-                    for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
-                    const double fn = fma(c, fb[j], -fa[j]);
-                    fa[j] = fb[j];
-                    fb[j] = fn;
-                }
+            for (int q = 0; q < NSRC; ++q) {
+                const double tot = warp_transpose_reduce<V>(acc[q], lane);
+                if ((lane & (32 / V - 1)) == 0) rb[q * V + lane / (32 / V)] = tot;
             }
         } else {
-            // ---- ragged top: skip slots that have not started, predicate single lanes
-#pragma unroll
-            for (int j = 0; j < T; ++j) {
-                if (j < nslot && __any_sync(FULL, t >= tp[j])) {
-                    if (t >= tp[j]) {
-#pragma unroll
-                        for (int s = 0; s < V; ++s) {
-                            const double c = (tl0 - 2.0 * s) * ix[j];
-#pragma unroll
-                            for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
-                            const double fn = fma(c, fb[j], -fa[j]);
-                            fa[j] = fb[j];
-                            fb[j] = fn;
-                        }
+            for (int idx = lane; idx < NSRC * V; idx += 32) rb[idx] = 0.0;
+        }
+
+        if (++g == G || t == p.n_tiles - 1) {
+            // ---- flush: warps summed in fixed order, Delta^E prefactor, store
+            __syncthreads();
+            const double *fbuf = ring + (size_t)phase * G * W * NSRC * V;
+            for (int idx = tid; idx < g * NSRC * V; idx += blockDim.x) {
+                const int gi = idx / (NSRC * V), r = idx - gi * (NSRC * V);
+                const int q = r / V, s = r - q * V;
+                const int l = p.l_max - (t_flush + gi) * V - s;
+                if (l >= p.l_min) {
+                    const int li = p.l_index[l];
+                    if (li >= 0) {
+                        double sum = 0.0;
+                        for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * NSRC * V + r];
+                        if (q == 1) sum *= p.pref[li];
+                        double *dst = p.Delta + (delta_b + (size_t)q * p.n_l + li) * p.n_k + kidx;
+                        if (p.n_split == 1) *dst = sum;
+                        else atomicAdd(dst, sum);
                     }
                 }
             }
+            phase ^= 1;
+            g = 0;
+            t_flush = t + 1;
         }
-
-        // ---- cross-thread reduction: warp butterfly, then warps through shared memory
-        double *rb = red + (size_t)buf * W * NSRC * V;
-#pragma unroll
-        for (int q = 0; q < NSRC; ++q) {
-            const double tot = warp_transpose_reduce<V>(acc[q], lane);
-            if ((lane & (32 / V - 1)) == 0) rb[(warp * NSRC + q) * V + lane / (32 / V)] = tot;
-        }
-        __syncthreads();
-        for (int idx = tid; idx < NSRC * V; idx += blockDim.x) {
-            const int q = idx / V, s = idx - q * V;
-            const int l = lhi - s;
-            if (l >= p.l_min) {
-                const int li = p.l_index[l];
-                if (li >= 0) {
-                    double sum = 0.0;
-                    for (int wv = 0; wv < W; ++wv) sum += rb[(wv * NSRC + q) * V + s];
-                    if (q == 1) sum *= p.pref[li];
-                    double *dst = p.Delta + (delta_b + (size_t)q * p.n_l + li) * p.n_k + kidx;
-                    if (p.n_split == 1) *dst = sum;
-                    else atomicAdd(dst, sum);
-                }
-            }
-        }
-        buf ^= 1;
     }
 }
 
 // ------------------------------------------------------------------------------------------
+constexpr int RING_G = 8;   // tiles between CTA-wide flushes
+
+// CTA sizes are powers of two of warps (1, 2, 4, 8): the hardware deals a CTA's warps round-robin
+// to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA advances at the pace of
+// its slowest warp, so warp counts such as 5 leave one pipe with twice the work of the others
+// (measured: profiles/README.md).  T is then the smallest slot count that covers the tau range.
 TransferShape choose_shape(int n_tau, int n_src)
 {
     TransferShape s;
-    s.T = 8;
     s.V = n_src == 2 ? 16 : 8;
-    const int max_threads = n_src == 2 ? 384 : 320;   // register file: threads * regs <= 64K
+    const int t_max = 8;
     s.n_split = 1;
     for (;;) {
         const int len = (n_tau + s.n_split - 1) / s.n_split;
-        const int threads = ((len + s.T - 1) / s.T + 31) / 32 * 32;
-        if (threads <= max_threads) { s.threads = threads; break; }
+        int best_pad = 0x7fffffff;
+        for (int threads = 256; threads >= 32; threads >>= 1) {
+            const int T = (len + threads - 1) / threads;
+            if (T > t_max) break;
+            const int pad = T * threads - len;
+            // prefer less padding; at equal padding the larger CTA (fewer, longer chains per thread)
+            if (T >= 3 && pad < best_pad) { best_pad = pad; s.threads = threads; s.T = T; }
+            if (T < 3 && best_pad == 0x7fffffff) { best_pad = pad; s.threads = threads; s.T = T; }
+        }
+        if (best_pad != 0x7fffffff) break;
         ++s.n_split;
     }
     return s;
 }
 
-template <int T, int V, int NSRC, int MAXT, int MINB>
+template <int T, int V, int NSRC>
 static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &sh, cudaStream_t stream)
 {
     dim3 grid((unsigned)(prm.n_k * prm.n_batch), (unsigned)sh.n_split);
-    const size_t smem = sizeof(double) * 2 * (sh.threads / 32) * NSRC * V;
-    transfer_kernel<T, V, NSRC, MAXT, MINB><<<grid, sh.threads, smem, stream>>>(prm);
+    const int W = sh.threads / 32;
+    const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * 2 * RING_G * W * NSRC * V +
+                        sizeof(int) * W * T;
+    auto kern = transfer_kernel<T, V, NSRC, RING_G, 256, (T <= 5 && NSRC == 2) ? 2 : 1>;
+    if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
+        GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, sh.threads, smem, stream>>>(prm);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
+}
+
+template <int V, int NSRC>
+static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, cudaStream_t stream)
+{
+    switch (sh.T) {
+    case 1: return launch_impl<1, V, NSRC>(prm, sh, stream);
+    case 2: return launch_impl<2, V, NSRC>(prm, sh, stream);
+    case 3: return launch_impl<3, V, NSRC>(prm, sh, stream);
+    case 4: return launch_impl<4, V, NSRC>(prm, sh, stream);
+    case 5: return launch_impl<5, V, NSRC>(prm, sh, stream);
+    case 6: return launch_impl<6, V, NSRC>(prm, sh, stream);
+    case 7: return launch_impl<7, V, NSRC>(prm, sh, stream);
+    case 8: return launch_impl<8, V, NSRC>(prm, sh, stream);
+    }
+    set_error("no transfer kernel for T=%d", sh.T);
+    return GCAMB_EINVAL;
 }
 
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
@@ -230,9 +294,9 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
         const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
         GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
     }
-    if (p->n_src == 2 && sh.T == 8 && sh.V == 16) return launch_impl<8, 16, 2, 384, 1>(prm, sh, stream);
-    if (p->n_src == 3 && sh.T == 8 && sh.V == 8) return launch_impl<8, 8, 3, 320, 1>(prm, sh, stream);
-    set_error("no transfer kernel for T=%d V=%d n_src=%d", sh.T, sh.V, p->n_src);
+    if (p->n_src == 2 && sh.V == 16) return launch_T<16, 2>(prm, sh, stream);
+    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, stream);
+    set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
     return GCAMB_EINVAL;
 }
 
