@@ -15,8 +15,8 @@
 // tile body is instantiated for every number NA of started slots (warp-uniform), so slots that
 // have not started cost nothing and started ones always run as NA interleaved chains.
 //
-// Reduction: after a tile the V x n_src per-thread sums are reduced across the warp with a
-// transposing butterfly (1 DADD + 1 double SHFL per l and source) into a shared-memory ring;
+// Reduction: after a tile the V x n_src per-thread sums are reduced across the warp through a
+// shared-memory transpose (1 DADD per l and source, no shuffles or selects) into a ring;
 // every G tiles the CTA synchronises once, sums the warps in fixed order, applies the Delta^E
 // prefactor and stores.  The summation order is fixed by the launch shape alone, so results are
 // bit-reproducible and the batched call equals a loop of single calls.
@@ -36,25 +36,28 @@ struct TransferParams {
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int NEVER = 0x7fffffff;
 
-// a[s] (s < V) per lane  ->  sum over the 32 lanes of a[s], returned on every lane for
-// s = lane / (32 / V).  V/2 + V/4 + ... + 1 exchanges, then log2(32/V) plain butterfly steps.
-template <int V>
-__device__ __forceinline__ double warp_transpose_reduce(double (&a)[V], int lane)
+// Cross-lane reduction of one tile: every lane holds P = NSRC*V partial sums (acc flattened as
+// [q][s]); lane c < P returns the sum over the 32 lanes of partial c, added in lane order.
+// Transposed through a per-warp shared-memory scratch [32][P+2] (the +2 keeps the 16-byte stores
+// of a quarter-warp on distinct banks): P/2 STS.128 + 32 LDS.64 + 31 DADD per lane, against
+// ~9 issue slots per partial for a shuffle butterfly -- on sm_100a an FP64 instruction holds its
+// sub-partition's issue port for two cycles and nothing co-issues with it, so every other
+// instruction costs FP64 time (profiles/README.md, "machine model").
+template <int P>
+__device__ __forceinline__ double warp_transpose_reduce(const double *vals, double *scratch, int lane)
 {
-    int bit = 16;
+    constexpr int RS = P + 2;
+    double2 *row = reinterpret_cast<double2 *>(scratch + lane * RS);
 #pragma unroll
-    for (int h = V / 2; h >= 1; h >>= 1, bit >>= 1) {
-        const bool up = (lane & bit) != 0;
+    for (int i = 0; i < P / 2; ++i) row[i] = make_double2(vals[2 * i], vals[2 * i + 1]);
+    __syncwarp();
+    double sum = 0.0;
+    if (lane < P) {
 #pragma unroll
-        for (int i = 0; i < h; ++i) {
-            const double send = up ? a[i] : a[i + h];
-            const double keep = up ? a[i + h] : a[i];
-            a[i] = keep + __shfl_xor_sync(FULL, send, bit);
-        }
+        for (int r = 0; r < 32; ++r) sum += scratch[r * RS + lane];
     }
-#pragma unroll
-    for (; bit >= 1; bit >>= 1) a[0] += __shfl_xor_sync(FULL, a[0], bit);
-    return a[0];
+    __syncwarp();
+    return sum;
 }
 
 // a2 + a3 for one l-tile and the first NA slots of this thread: NA independent recurrence chains.
@@ -81,11 +84,14 @@ template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
     static_assert(T >= 1 && T <= 10, "the NA dispatch below is written out for T <= 10");
-    extern __shared__ double2 smem2[];   // start pairs [T][threads], ring [2][G][W][NSRC][V], slot starts [W][T]
+    constexpr int P = NSRC * V;          // partial sums per thread and tile
+    // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] | slot starts [W][T]
+    extern __shared__ double2 smem2[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
     double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
-    double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x);
-    int *slot_start = reinterpret_cast<int *>(ring + (size_t)2 * G * W * NSRC * V);
+    double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)warp * 32 * (P + 2);
+    double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
+    int *slot_start = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P);
     const int bid = blockIdx.x;
     const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;
     const int kidx = p.korder[krank];
@@ -96,11 +102,14 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const size_t row = (size_t)kidx * p.n_tau;
 
     // ---- a1: source staging.  Slot j of the CTA covers tau indices i_begin + j*blockDim ...
-    // + blockDim - 1, dealt round-robin to the warps (lane*W + warp) so that every warp sees the
-    // same mix of start tiles and the warps of a CTA stay in step between flushes.
+    // + blockDim - 1 in W chunks of 32 consecutive tau ("ranks"; rank 0 has the largest x and the
+    // most work).  A warp keeps one rank for all its slots, so its lanes start within a tile or two
+    // of each other (lockstep waste ~1%); the rank -> warp map rotates with the CTA index so that
+    // the heavy ranks of co-resident CTAs land on different sub-partitions.
     double fa[T], fb[T], ix[T], src[NSRC][T];
     int tp[T];
-    const int i_mine = i_begin + lane * W + warp;
+    const int rank = (warp + bid) % W;
+    const int i_mine = i_begin + rank * 32 + lane;
 #pragma unroll
     for (int j = 0; j < T; ++j) {
         const int i = i_mine + j * (int)blockDim.x;
@@ -163,7 +172,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             }
         }
 
-        double *rb = ring + ((size_t)(phase * G + g) * W + warp) * NSRC * V;
+        double *rb = ring + ((size_t)(phase * G + g) * W + rank) * P;   // by rank: fixed summation order
         if (na > 0) {
             const double tl0 = (double)(2 * (p.l_max - t * V) + 1);
             double acc[NSRC][V];
@@ -178,11 +187,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             }
 #undef GCAMB_NA
             // cross-lane reduction into this warp's ring entry
-#pragma unroll
-            for (int q = 0; q < NSRC; ++q) {
-                const double tot = warp_transpose_reduce<V>(acc[q], lane);
-                if ((lane & (32 / V - 1)) == 0) rb[q * V + lane / (32 / V)] = tot;
-            }
+            const double tot = warp_transpose_reduce<P>(&acc[0][0], scratch, lane);
+            if (lane < P) rb[lane] = tot;
         } else {
             for (int idx = lane; idx < NSRC * V; idx += 32) rb[idx] = 0.0;
         }
@@ -225,18 +231,18 @@ TransferShape choose_shape(int n_tau, int n_src)
 {
     TransferShape s;
     s.V = n_src == 2 ? 16 : 8;
-    const int t_max = 8;
+    const int t_max = 10;
     s.n_split = 1;
     for (;;) {
         const int len = (n_tau + s.n_split - 1) / s.n_split;
         int best_pad = 0x7fffffff;
-        for (int threads = 256; threads >= 32; threads >>= 1) {
+        // least padding wins; at equal padding the smaller CTA, i.e. more points per thread: the
+        // cross-thread reduction costs one DADD per thread, tile row and source whatever T is
+        for (int threads = 32; threads <= 256; threads <<= 1) {
             const int T = (len + threads - 1) / threads;
-            if (T > t_max) break;
+            if (T > t_max) continue;
             const int pad = T * threads - len;
-            // prefer less padding; at equal padding the larger CTA (fewer, longer chains per thread)
-            if (T >= 3 && pad < best_pad) { best_pad = pad; s.threads = threads; s.T = T; }
-            if (T < 3 && best_pad == 0x7fffffff) { best_pad = pad; s.threads = threads; s.T = T; }
+            if (pad < best_pad) { best_pad = pad; s.threads = threads; s.T = T; }
         }
         if (best_pad != 0x7fffffff) break;
         ++s.n_split;
@@ -249,9 +255,9 @@ static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &
 {
     dim3 grid((unsigned)(prm.n_k * prm.n_batch), (unsigned)sh.n_split);
     const int W = sh.threads / 32;
-    const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * 2 * RING_G * W * NSRC * V +
-                        sizeof(int) * W * T;
-    auto kern = transfer_kernel<T, V, NSRC, RING_G, 256, (T <= 5 && NSRC == 2) ? 2 : 1>;
+    const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
+                        sizeof(double) * 2 * RING_G * W * NSRC * V + sizeof(int) * W * T;
+    auto kern = transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
     if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, sh.threads, smem, stream>>>(prm);
@@ -271,6 +277,8 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
     case 6: return launch_impl<6, V, NSRC>(prm, sh, stream);
     case 7: return launch_impl<7, V, NSRC>(prm, sh, stream);
     case 8: return launch_impl<8, V, NSRC>(prm, sh, stream);
+    case 9: return launch_impl<9, V, NSRC>(prm, sh, stream);
+    case 10: return launch_impl<10, V, NSRC>(prm, sh, stream);
     }
     set_error("no transfer kernel for T=%d", sh.T);
     return GCAMB_EINVAL;
