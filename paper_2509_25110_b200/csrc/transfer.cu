@@ -37,25 +37,39 @@ constexpr unsigned FULL = 0xffffffffu;
 constexpr int NEVER = 0x7fffffff;
 
 // Cross-lane reduction of one tile: every lane holds P = NSRC*V partial sums (acc flattened as
-// [q][s]); lane c < P returns the sum over the 32 lanes of partial c, added in lane order.
+// [q][s]); lane c < P returns the sum over the 32 lanes of partial c, in a fixed order.
 // Transposed through a per-warp shared-memory scratch [32][P+2] (the +2 keeps the 16-byte stores
-// of a quarter-warp on distinct banks): P/2 STS.128 + 32 LDS.64 + 31 DADD per lane, against
-// ~9 issue slots per partial for a shuffle butterfly -- on sm_100a an FP64 instruction holds its
-// sub-partition's issue port for two cycles and nothing co-issues with it, so every other
-// instruction costs FP64 time (profiles/README.md, "machine model").
+// of a quarter-warp on distinct banks).  With C = the power of two >= P, the warp splits into
+// 32/C lane groups; group g sums rows g*C .. g*C+C-1 of column lane%C in two interleaved chains
+// (DADD latency, not throughput, bounds a single chain), then the groups are combined by xor
+// shuffles: P/2 STS.128 + C LDS.64 + (C + log2(32/C)) DADD per lane, against ~9 issue slots per
+// partial for a shuffle butterfly -- on sm_100a an FP64 instruction holds its sub-partition's
+// issue port for two cycles and nothing co-issues with it, so every other instruction costs
+// FP64 time (profiles/README.md, "machine model").
 template <int P>
 __device__ __forceinline__ double warp_transpose_reduce(const double *vals, double *scratch, int lane)
 {
     constexpr int RS = P + 2;
+    constexpr int C = P <= 8 ? 8 : (P <= 16 ? 16 : 32);   // columns per lane group
+    constexpr int ROWS = C;                               // rows per lane group = 32 / (32 / C)
+    static_assert(P <= 32 && P % 2 == 0, "one column per lane");
     double2 *row = reinterpret_cast<double2 *>(scratch + lane * RS);
 #pragma unroll
     for (int i = 0; i < P / 2; ++i) row[i] = make_double2(vals[2 * i], vals[2 * i + 1]);
     __syncwarp();
-    double sum = 0.0;
-    if (lane < P) {
+    const int col = lane & (C - 1), grp = lane / C;
+    double s0 = 0.0, s1 = 0.0;
+    if (col < P) {
+        const double *base = scratch + (size_t)grp * ROWS * RS + col;
 #pragma unroll
-        for (int r = 0; r < 32; ++r) sum += scratch[r * RS + lane];
+        for (int r = 0; r < ROWS; r += 2) {
+            s0 += base[r * RS];
+            s1 += base[(r + 1) * RS];
+        }
     }
+    double sum = s0 + s1;
+#pragma unroll
+    for (int o = C; o < 32; o <<= 1) sum += __shfl_xor_sync(FULL, sum, o);
     __syncwarp();
     return sum;
 }
@@ -222,6 +236,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 
 // ------------------------------------------------------------------------------------------
 constexpr int RING_G = 8;   // tiles between CTA-wide flushes
+#ifndef GCAMB_MINB
+#define GCAMB_MINB 3
+#endif
+#ifndef GCAMB_V2
+#define GCAMB_V2 8          // l-tile for n_src = 2
+#endif
 
 // CTA sizes are powers of two of warps (1, 2, 4, 8): the hardware deals a CTA's warps round-robin
 // to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA advances at the pace of
@@ -230,7 +250,7 @@ constexpr int RING_G = 8;   // tiles between CTA-wide flushes
 TransferShape choose_shape(int n_tau, int n_src)
 {
     TransferShape s;
-    s.V = n_src == 2 ? 16 : 8;
+    s.V = n_src == 2 ? GCAMB_V2 : 8;
     const int t_max = 10;
     s.n_split = 1;
     for (;;) {
@@ -257,7 +277,9 @@ static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &
     const int W = sh.threads / 32;
     const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
                         sizeof(double) * 2 * RING_G * W * NSRC * V + sizeof(int) * W * T;
-    auto kern = transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
+    // register budget: CTAs of <= 128 threads are compiled for GCAMB_MINB co-resident CTAs per SM
+    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB>
+                                  : transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
     if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, sh.threads, smem, stream>>>(prm);
@@ -302,7 +324,7 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
         const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
         GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
     }
-    if (p->n_src == 2 && sh.V == 16) return launch_T<16, 2>(prm, sh, stream);
+    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, stream);
     if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, stream);
     set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
     return GCAMB_EINVAL;
