@@ -51,7 +51,7 @@ static void free_plan(gcamb_los_plan *p)
     if (!p) return;
     cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
     cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile);
-    cudaFree(p->d_korder);
+    cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     delete p;
@@ -130,6 +130,7 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
 
     cudaError_t e = cudaGetDevice(&p->device);
     if (e == cudaSuccess) e = upload(&p->d_l_index, l_index, stream);
+    if (e == cudaSuccess) e = upload(&p->d_l_list, std::vector<int32_t>(l_list, l_list + n_l), stream);
     if (e == cudaSuccess) e = upload(&p->d_k, vk, stream);
     if (e == cudaSuccess) e = upload(&p->d_chi, chi, stream);
     if (e == cudaSuccess) e = upload(&p->d_w, w, stream);

@@ -38,6 +38,8 @@ struct gcamb_los_plan {
     double2 *d_start;    // [n_k][n_tau] (j_{lhi+1}(x), j_{lhi}(x)), lhi = l_max - V*tile
     int32_t *d_tile;     // [n_k][n_tau] first l-tile of the point
     int32_t *d_korder;   // [n_k] k indices, heaviest first
+    int32_t *d_l_list;   // [n_l] the l list
+    int32_t *d_kz;       // [n_tiles] #k whose walk starts below tile t: Delta rows of tile t are 0 for k < kz[t]; NULL if not monotone
 
     // scratch of gcamb_los_spectra_host (lazily allocated)
     int32_t host_batch_cap;

@@ -91,7 +91,8 @@ __global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ 
                                                      int l_min, int l_max, int V,
                                                      const int32_t *__restrict__ tile,
                                                      long long *__restrict__ walked,
-                                                     long long *__restrict__ executed)
+                                                     long long *__restrict__ executed,
+                                                     long long *__restrict__ first_tile)
 {
     __shared__ long long sw[256], se[256];
     const int j = blockIdx.x;
@@ -113,7 +114,7 @@ __global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ 
         }
         __syncthreads();
     }
-    if (threadIdx.x == 0) { walked[j] = sw[0]; executed[j] = se[0]; }
+    if (threadIdx.x == 0) { walked[j] = sw[0]; executed[j] = se[0]; first_tile[j] = tile[(size_t)j * n_tau]; }
 }
 
 gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
@@ -125,11 +126,11 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     GCAMB_CUDA(cudaGetLastError());
 
     long long *d_cost = nullptr;
-    GCAMB_CUDA(cudaMalloc(&d_cost, sizeof(long long) * 2 * (size_t)p->n_k));
+    GCAMB_CUDA(cudaMalloc(&d_cost, sizeof(long long) * 3 * (size_t)p->n_k));
     k_cost_kernel<<<p->n_k, 256, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_min, p->l_max, V,
-                                              p->d_tile, d_cost, d_cost + p->n_k);
+                                              p->d_tile, d_cost, d_cost + p->n_k, d_cost + 2 * p->n_k);
     cudaError_t e = cudaGetLastError();
-    std::vector<long long> cost(2 * (size_t)p->n_k);
+    std::vector<long long> cost(3 * (size_t)p->n_k);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(cost.data(), d_cost, sizeof(long long) * cost.size(),
                             cudaMemcpyDeviceToHost, stream);
@@ -138,7 +139,7 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     if (e != cudaSuccess) return cuda_fail(e, "plan precompute");
 
     p->walked_terms = std::accumulate(cost.begin(), cost.begin() + p->n_k, 0LL);
-    p->executed_terms = std::accumulate(cost.begin() + p->n_k, cost.end(), 0LL);
+    p->executed_terms = std::accumulate(cost.begin() + p->n_k, cost.begin() + 2 * p->n_k, 0LL);
     // heaviest k first: the CTA scheduler hands out blockIdx in order (longest-processing-time rule)
     std::vector<int32_t> order(p->n_k);
     std::iota(order.begin(), order.end(), 0);
@@ -146,6 +147,23 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
                      [&](int32_t a, int32_t b) { return cost[a] > cost[b]; });
     GCAMB_CUDA(cudaMemcpyAsync(p->d_korder, order.data(), sizeof(int32_t) * p->n_k,
                                cudaMemcpyHostToDevice, stream));
+    // zero region of Delta (R16): x grows with k, so the first tile of a k (that of tau_0, its
+    // largest x) never rises with k, and the rows of tile t are exactly zero for the first kz[t]
+    // k.  If the first tiles were ever not monotone the kernel falls back to per-CTA zero stores.
+    const long long *first = cost.data() + 2 * (size_t)p->n_k;
+    bool monotone = true;
+    for (int j = 1; j < p->n_k; ++j) monotone = monotone && first[j] <= first[j - 1];
+    p->d_kz = nullptr;
+    if (monotone) {
+        std::vector<int32_t> kz(p->n_tiles);
+        int j = p->n_k;   // kz[t] = #{k : first[k] > t}, non-increasing in t
+        for (int t = 0; t < p->n_tiles; ++t) {
+            while (j > 0 && first[j - 1] <= t) --j;
+            kz[t] = j;
+        }
+        GCAMB_CUDA(cudaMalloc(&p->d_kz, sizeof(int32_t) * p->n_tiles));
+        GCAMB_CUDA(cudaMemcpyAsync(p->d_kz, kz.data(), sizeof(int32_t) * p->n_tiles, cudaMemcpyHostToDevice, stream));
+    }
     GCAMB_CUDA(cudaStreamSynchronize(stream));
     return GCAMB_OK;
 }

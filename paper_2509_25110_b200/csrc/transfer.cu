@@ -29,8 +29,9 @@ struct TransferParams {
     double *Delta;
     const double *k, *chi, *w, *pref;
     const double2 *start;
-    const int32_t *tile, *korder, *l_index;
+    const int32_t *tile, *korder, *l_index, *l_list, *kz;
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
+    int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
 };
 
 constexpr unsigned FULL = 0xffffffffu;
@@ -99,13 +100,16 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 {
     static_assert(T >= 1 && T <= 10, "the NA dispatch below is written out for T <= 10");
     constexpr int P = NSRC * V;          // partial sums per thread and tile
-    // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] | slot starts [W][T]
+    constexpr int NOUT = (G * P + MAXTHREADS - 1) / MAXTHREADS;   // flush outputs per thread (full CTA)
+    // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] |
+    // start tiles [T][threads] | slot first/last start tile [W][2T]
     extern __shared__ double2 smem2[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
     double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
     double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)warp * 32 * (P + 2);
     double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
-    int *slot_start = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P);
+    int *my_tile = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + tid;   // [j * blockDim]
+    int *slot_win = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + (size_t)T * blockDim.x + warp * 2 * T;
     const int bid = blockIdx.x;
     const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;
     const int kidx = p.korder[krank];
@@ -121,74 +125,115 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // of each other (lockstep waste ~1%); the rank -> warp map rotates with the CTA index so that
     // the heavy ranks of co-resident CTAs land on different sub-partitions.
     double fa[T], fb[T], ix[T], src[NSRC][T];
-    int tp[T];
     const int rank = (warp + bid) % W;
     const int i_mine = i_begin + rank * 32 + lane;
 #pragma unroll
     for (int j = 0; j < T; ++j) {
         const int i = i_mine + j * (int)blockDim.x;
         fa[j] = fb[j] = 0.0;
+        int tp = NEVER;
         if (i < i_end) {
             const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + i;
             const double x = __dmul_rn(kval, p.chi[i]);
             const double inv = 1.0 / x;
             const double w = p.w[i];
             ix[j] = inv;
-            tp[j] = p.tile[row + i];
+            tp = p.tile[row + i];
             my_start[j * blockDim.x] = p.start[row + i];
             src[0][j] = w * p.S[0][sx];
             src[1][j] = w * p.S[1][sx] * (inv * inv);
             if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
         } else {
             ix[j] = 0.0;
-            tp[j] = NEVER;
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) src[q][j] = 0.0;
         }
-        // x falls with tau: the slot starts with its first lane, and slot j never before slot j-1
-        const int first = __reduce_min_sync(FULL, tp[j]);
-        if (lane == 0) slot_start[warp * T + j] = first;
+        my_tile[j * blockDim.x] = tp;
+        // x falls with tau: within a warp every point of slot j starts no later than any point of
+        // slot j+1, so the start windows [first, last] of the slots are ordered
+        const int first = __reduce_min_sync(FULL, tp);
+        const int last = __reduce_max_sync(FULL, tp == NEVER ? -1 : tp);
+        if (lane == 0) { slot_win[2 * j] = first; slot_win[2 * j + 1] = last; }
     }
     __syncwarp();
 
     // first tile of this CTA = start tile of its largest x
     const int t_begin = p.tile[row + i_begin];
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
+#define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
 
-    // l above the first tile: Delta is exactly zero there (R16).  With RED output the buffer was
-    // zeroed by the launcher instead.
+    // l above the first tile of a k: Delta is exactly zero there (R16).  Those elements form, for
+    // every l, a prefix k < kz[tile of l] of the Delta row, so the CTAs share the rows among
+    // themselves and zero them with coalesced stores (a CTA's own zero elements lie along l, 8 bytes
+    // every n_k doubles).  With RED output the launcher zeroed the whole buffer instead.
     if (p.n_split == 1) {
-        const int l_top = p.l_max - t_begin * V;  // highest l walked
-        for (int l = p.l_max - tid; l > l_top; l -= blockDim.x) {
-            const int li = p.l_index[l];
-            if (li >= 0) {
+        if (p.kz) {
+            const int n_rows = NSRC * p.n_l;
+            for (int r = krank; r < n_rows; r += gridDim.x / p.n_batch) {
+                const int li = r % p.n_l;
+                const int nz = p.kz[(p.l_max - p.l_list[li]) / V];
+                double *dst = p.Delta + (delta_b + r) * p.n_k;
+                for (int j = tid; j < nz; j += blockDim.x) dst[j] = 0.0;
+            }
+        } else {
+            const int l_top = max(p.l_max - t_begin * V, p.l_min - 1);  // highest l walked
+            for (int l = p.l_max - tid; l > l_top; l -= blockDim.x) {
+                const int li = p.l_contig ? l - p.l_min : p.l_index[l];
+                if (li >= 0) {
 #pragma unroll
-                for (int q = 0; q < NSRC; ++q) p.Delta[(delta_b + (size_t)q * p.n_l + li) * p.n_k + kidx] = 0.0;
+                    for (int q = 0; q < NSRC; ++q) p.Delta[DIDX(q, li)] = 0.0;
+                }
             }
         }
     }
 
+    // flush bookkeeping: output `o` of this thread in a G-tile group is ring column
+    // idx = tid + o*blockDim -> (tile gi, source q, row s); its l-index and Delta^E prefactor are
+    // fetched one group ahead so that the flush itself waits on no global load
+    int f_li[NOUT];
+    double f_pref[NOUT];
+    auto prefetch_flush = [&](int t_first) {
+#pragma unroll
+        for (int o = 0; o < NOUT; ++o) {
+            const int idx = tid + o * (int)blockDim.x;
+            const int gi = idx / P, r = idx - gi * P, q = r / V, s = r - q * V;
+            const int l = p.l_max - (t_first + gi) * V - s;
+            int li = -1;
+            if (idx < G * P && l >= p.l_min) li = p.l_contig ? l - p.l_min : p.l_index[l];
+            f_li[o] = li;
+            f_pref[o] = (q == 1 && li >= 0) ? p.pref[li] : 1.0;
+        }
+    };
+    prefetch_flush(t_begin);
+
     int na = 0;                               // started slots of this warp (warp-uniform)
-    int next_slot = slot_start[warp * T];     // tile at which slot `na` starts
+    int next_slot = slot_win[0];              // tile at which slot `na` starts
+    int inj = 0;                              // first slot with points still to start (warp-uniform)
+    int inj_from = slot_win[0];               // its first start tile
     int phase = 0, g = 0, t_flush = t_begin;  // ring bookkeeping (CTA-uniform)
-    for (int t = t_begin; t < p.n_tiles; ++t) {
+    double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);   // 2l+1 at the top of the tile
+    for (int t = t_begin; t < p.n_tiles; ++t, tl0 -= 2.0 * V) {
         while (next_slot <= t) {
             ++na;
-            next_slot = na < T ? slot_start[warp * T + na] : NEVER;
+            next_slot = na < T ? slot_win[2 * na] : NEVER;
         }
-        // inject the plan's start pair (j_{lhi+1}, j_lhi) into points whose walk begins here
+        // inject the plan's start pair (j_{lhi+1}, j_lhi) into points whose walk begins here;
+        // skipped (warp-uniformly) on the tiles where no slot of this warp is inside its window
+        if (inj_from <= t) {
 #pragma unroll
-        for (int j = 0; j < T; ++j) {
-            if (tp[j] == t) {
-                const double2 st = my_start[j * blockDim.x];
-                fa[j] = st.x;
-                fb[j] = st.y;
+            for (int j = 0; j < T; ++j) {
+                if (my_tile[j * blockDim.x] == t) {
+                    const double2 st = my_start[j * blockDim.x];
+                    fa[j] = st.x;
+                    fb[j] = st.y;
+                }
             }
+            while (inj < T && slot_win[2 * inj + 1] <= t) ++inj;
+            inj_from = inj < T ? slot_win[2 * inj] : NEVER;
         }
 
         double *rb = ring + ((size_t)(phase * G + g) * W + rank) * P;   // by rank: fixed summation order
         if (na > 0) {
-            const double tl0 = (double)(2 * (p.l_max - t * V) + 1);
             double acc[NSRC][V];
 #pragma unroll
             for (int q = 0; q < NSRC; ++q)
@@ -204,38 +249,54 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             const double tot = warp_transpose_reduce<P>(&acc[0][0], scratch, lane);
             if (lane < P) rb[lane] = tot;
         } else {
-            for (int idx = lane; idx < NSRC * V; idx += 32) rb[idx] = 0.0;
+            for (int idx = lane; idx < P; idx += 32) rb[idx] = 0.0;
         }
 
         if (++g == G || t == p.n_tiles - 1) {
             // ---- flush: warps summed in fixed order, Delta^E prefactor, store
             __syncthreads();
-            const double *fbuf = ring + (size_t)phase * G * W * NSRC * V;
-            for (int idx = tid; idx < g * NSRC * V; idx += blockDim.x) {
-                const int gi = idx / (NSRC * V), r = idx - gi * (NSRC * V);
-                const int q = r / V, s = r - q * V;
+            const double *fbuf = ring + (size_t)phase * G * W * P;
+#pragma unroll
+            for (int o = 0; o < NOUT; ++o) {
+                const int idx = tid + o * (int)blockDim.x;
+                const int li = f_li[o];
+                if (idx < g * P && li >= 0) {
+                    const int gi = idx / P, r = idx - gi * P, q = r / V;
+                    double sum = 0.0;
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    sum *= f_pref[o];
+                    double *dst = p.Delta + DIDX(q, li);
+                    if (p.n_split == 1) *dst = sum;
+                    else atomicAdd(dst, sum);
+                }
+            }
+            // CTAs smaller than the one NOUT was sized for: the remaining columns, unprefetched
+            for (int idx = tid + NOUT * (int)blockDim.x; idx < g * P; idx += blockDim.x) {
+                const int gi = idx / P, r = idx - gi * P, q = r / V, s = r - q * V;
                 const int l = p.l_max - (t_flush + gi) * V - s;
-                if (l >= p.l_min) {
-                    const int li = p.l_index[l];
-                    if (li >= 0) {
-                        double sum = 0.0;
-                        for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * NSRC * V + r];
-                        if (q == 1) sum *= p.pref[li];
-                        double *dst = p.Delta + (delta_b + (size_t)q * p.n_l + li) * p.n_k + kidx;
-                        if (p.n_split == 1) *dst = sum;
-                        else atomicAdd(dst, sum);
-                    }
+                const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
+                if (li >= 0) {
+                    double sum = 0.0;
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    if (q == 1) sum *= p.pref[li];
+                    double *dst = p.Delta + DIDX(q, li);
+                    if (p.n_split == 1) *dst = sum;
+                    else atomicAdd(dst, sum);
                 }
             }
             phase ^= 1;
             g = 0;
             t_flush = t + 1;
+            prefetch_flush(t_flush);
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------
-constexpr int RING_G = 8;   // tiles between CTA-wide flushes
+#ifndef GCAMB_G
+#define GCAMB_G 8
+#endif
+constexpr int RING_G = GCAMB_G;   // tiles between CTA-wide flushes
 #ifndef GCAMB_MINB
 #define GCAMB_MINB 3
 #endif
@@ -276,7 +337,8 @@ static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &
     dim3 grid((unsigned)(prm.n_k * prm.n_batch), (unsigned)sh.n_split);
     const int W = sh.threads / 32;
     const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
-                        sizeof(double) * 2 * RING_G * W * NSRC * V + sizeof(int) * W * T;
+                        sizeof(double) * 2 * RING_G * W * NSRC * V + sizeof(int) * T * sh.threads +
+                        sizeof(int) * W * 2 * T;
     // register budget: CTAs of <= 128 threads are compiled for GCAMB_MINB co-resident CTAs per SM
     auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB>
                                   : transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
@@ -316,9 +378,11 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
     prm.Delta = Delta;
     prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref;
     prm.start = p->d_start; prm.tile = p->d_tile; prm.korder = p->d_korder; prm.l_index = p->d_l_index;
+    prm.l_list = p->d_l_list; prm.kz = p->d_kz;
     prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l;
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
+    prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
     if (sh.n_split > 1) {
         const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
