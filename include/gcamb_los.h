@@ -87,6 +87,14 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
                                  int64_t *executed_terms);
 
 /*
+ * Kernels of this library that one gcamb_los_transfer[_batched] call and one gcamb_los_cls[_batched]
+ * call launch on this plan (any batch size; a cudaMemsetAsync of Delta precedes the transfer kernel
+ * when the tau grid is split over several CTAs per k).  Either pointer may be NULL.
+ */
+gcamb_status gcamb_los_plan_launches(const gcamb_los_plan *plan, int32_t *transfer_kernels,
+                                     int32_t *cls_kernels);
+
+/*
  * Eq. 2-3: sources -> transfer functions (steps a1-a3: source staging, j_l recurrence in
  * registers, tau-integration, cross-thread reduction, Delta^E prefactor).  Asynchronous on
  * `cuda_stream`; no allocation, no host<->device copy.

@@ -172,6 +172,14 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
     return GCAMB_OK;
 }
 
+gcamb_status gcamb_los_plan_launches(const gcamb_los_plan *plan, int32_t *transfer_kernels, int32_t *cls_kernels)
+{
+    if (!plan) { set_error("null plan"); return GCAMB_EINVAL; }
+    if (transfer_kernels) *transfer_kernels = 1;
+    if (cls_kernels) *cls_kernels = 1;
+    return GCAMB_OK;
+}
+
 gcamb_status gcamb_los_transfer_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,
                                         const double *d_S_E, const double *d_S_phi, double *d_Delta,
                                         void *cuda_stream)

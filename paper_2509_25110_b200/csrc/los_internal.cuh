@@ -25,6 +25,7 @@ struct gcamb_los_plan {
     double tau0;
     gcamb::TransferShape shape;
     int64_t executed_terms;  // sum over (k,tau) of #l in [l_min, min(L(x), l_max)]
+    int32_t n_comp;          // leading positions of korder that run the compensated coefficient (transfer.cu)
     int64_t walked_terms;    // same with the tile-aligned start the kernel really walks
     int device;
 
@@ -61,6 +62,12 @@ gcamb_status cuda_fail(cudaError_t e, const char *what);
 gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream);
 
 // transfer.cu
+// x above which the systematic phase error x 2^-53 of the rounded reciprocal exceeds 7.5e-13 rad
+//
+#ifndef GCAMB_COMP_X_MIN
+#define GCAMB_COMP_X_MIN 6755.399441055744   // 2^53 * 7.5e-13
+#endif
+constexpr double COMP_X_MIN = GCAMB_COMP_X_MIN;
 TransferShape choose_shape(int n_tau, int n_src);
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,

@@ -143,10 +143,25 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     // heaviest k first: the CTA scheduler hands out blockIdx in order (longest-processing-time rule)
     std::vector<int32_t> order(p->n_k);
     std::iota(order.begin(), order.end(), 0);
+    // ties (saturated rows) by k, so that the order is the k grid reversed whenever cost grows with k
     std::stable_sort(order.begin(), order.end(),
-                     [&](int32_t a, int32_t b) { return cost[a] > cost[b]; });
+                     [&](int32_t a, int32_t b) { return cost[a] != cost[b] ? cost[a] > cost[b] : a > b; });
     GCAMB_CUDA(cudaMemcpyAsync(p->d_korder, order.data(), sizeof(int32_t) * p->n_k,
                                cudaMemcpyHostToDevice, stream));
+    // rows whose largest x = k chi_max exceeds COMP_X_MIN run the compensated coefficient; they
+    // must be a prefix of the cost order (they are whenever cost grows with k), else all rows do
+    {
+        std::vector<double> hk(p->n_k);
+        double chi_max = 0.0;
+        GCAMB_CUDA(cudaMemcpyAsync(hk.data(), p->d_k, sizeof(double) * p->n_k, cudaMemcpyDeviceToHost, stream));
+        GCAMB_CUDA(cudaMemcpyAsync(&chi_max, p->d_chi, sizeof(double), cudaMemcpyDeviceToHost, stream));   // tau grows: chi_0 is the largest
+        GCAMB_CUDA(cudaStreamSynchronize(stream));
+        int n_comp = 0;
+        for (int j = 0; j < p->n_k; ++j) n_comp += hk[j] * chi_max > COMP_X_MIN;
+        bool prefix = true;
+        for (int r = 0; r < p->n_k; ++r) prefix = prefix && ((hk[order[r]] * chi_max > COMP_X_MIN) == (r < n_comp));
+        p->n_comp = prefix ? n_comp : p->n_k;
+    }
     // zero region of Delta (R16): x grows with k, so the first tile of a k (that of tau_0, its
     // largest x) never rises with k, and the rows of tile t are exactly zero for the first kz[t]
     // k.  If the first tiles were ever not monotone the kernel falls back to per-CTA zero stores.

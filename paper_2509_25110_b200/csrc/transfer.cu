@@ -32,6 +32,7 @@ struct TransferParams {
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
+    int n_comp;     // the first n_comp positions of korder (largest x) take the compensated coefficient
 };
 
 constexpr unsigned FULL = 0xffffffffu;
@@ -76,16 +77,29 @@ __device__ __forceinline__ double warp_transpose_reduce(const double *vals, doub
 }
 
 // a2 + a3 for one l-tile and the first NA slots of this thread: NA independent recurrence chains.
-template <int NA, int T, int V, int NSRC>
-__device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], const double (&src)[NSRC][T],
-                                          double (&fa)[T], double (&fb)[T], double (&acc)[NSRC][V])
+// Slots are taken one after the other (j outer, l inner): the V recurrence steps of a slot form
+// one dependent DFMA chain (8 cycles each, measured), which the 4-5 FP64 instructions of a step
+// and the other resident warps cover, and consecutive instructions share operands.
+//
+// COMP (reading R14): c = (2l+1) * fl(1/x) carries the relative
+// error r of the rounded reciprocal into EVERY step with the same sign, i.e. the walk follows
+// j_l(x (1 - r)): a phase error x r of up to x 2^-53 that the tau-sum's cancellation multiplies.
+// The compensated body adds the reciprocal's rounding residual: c = fma(2l+1, inv, e) with
+// e = (2l_top+1) * inv_lo taken once per tile (inv_lo ~ 1e-16 inv: its change inside a tile is
+// far below an ulp of c), which makes c the correctly rounded quotient.
+template <int NA, int T, int V, int NSRC, bool COMP>
+__device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], const double *ixlo, int stride,
+                                          const double (&src)[NSRC][T], double (&fa)[T], double (&fb)[T],
+                                          double (&acc)[NSRC][V])
 {
 #pragma unroll
-    for (int s = 0; s < V; ++s) {
-        const double tl = tl0 - 2.0 * s;   // 2l+1
+    for (int j = 0; j < NA; ++j) {
+        double e = 0.0;
+        if (COMP) e = tl0 * ixlo[j * stride];
 #pragma unroll
-        for (int j = 0; j < NA; ++j) {
-            const double c = tl * ix[j];
+        for (int s = 0; s < V; ++s) {
+            const double tl = tl0 - 2.0 * s;   // 2l+1
+            const double c = COMP ? fma(tl, ix[j], e) : tl * ix[j];
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
             const double fn = fma(c, fb[j], -fa[j]);
@@ -110,8 +124,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
     int *my_tile = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + tid;   // [j * blockDim]
     int *slot_win = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + (size_t)T * blockDim.x + warp * 2 * T;
+    // compensated rows only: residuals of the rounded reciprocals [T][threads], after the (8-byte aligned) int tables
+    double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) +
+                                                 (((size_t)T * blockDim.x + W * 2 * T + 1) & ~(size_t)1)) + tid;
     const int bid = blockIdx.x;
-    const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;
+    const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;   // krank: position in the cost order
+    const bool comp = krank < p.n_comp;   // CTA-uniform: this row takes the compensated coefficient
     const int kidx = p.korder[krank];
     const int split = blockIdx.y;
     const int i_begin = split * p.split_len;
@@ -121,15 +139,15 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 
     // ---- a1: source staging.  Slot j of the CTA covers tau indices i_begin + j*blockDim ...
     // + blockDim - 1 in W chunks of 32 consecutive tau ("ranks"; rank 0 has the largest x and the
-    // most work).  A warp keeps one rank for all its slots, so its lanes start within a tile or two
-    // of each other (lockstep waste ~1%); the rank -> warp map rotates with the CTA index so that
-    // the heavy ranks of co-resident CTAs land on different sub-partitions.
+    // most work: on the log-spaced part of the tau grid x halves across one slot).  The warps walk
+    // the tiles together, so the rank -> warp map rotates with the slot (not with the row: a row's
+    // result must not depend on where it sits in the launch) to give
+    // every warp the same mix of heavy and light ranks; the lanes of a warp slot are 32 consecutive
+    // tau and start within a tile or two of each other (lockstep waste ~1%).
     double fa[T], fb[T], ix[T], src[NSRC][T];
-    const int rank = (warp + bid) % W;
-    const int i_mine = i_begin + rank * 32 + lane;
 #pragma unroll
     for (int j = 0; j < T; ++j) {
-        const int i = i_mine + j * (int)blockDim.x;
+        const int i = i_begin + j * (int)blockDim.x + ((warp + j) % W) * 32 + lane;
         fa[j] = fb[j] = 0.0;
         int tp = NEVER;
         if (i < i_end) {
@@ -138,6 +156,10 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             const double inv = 1.0 / x;
             const double w = p.w[i];
             ix[j] = inv;
+            if (comp) {   // 1/x = inv + inv_lo,  inv_lo = -inv * (inv x - 1), the residual taken exactly by the fma
+                const double res = fma(inv, x, -1.0);
+                my_ixlo[j * blockDim.x] = -inv * res;
+            }
             tp = p.tile[row + i];
             my_start[j * blockDim.x] = p.start[row + i];
             src[0][j] = w * p.S[0][sx];
@@ -145,6 +167,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
         } else {
             ix[j] = 0.0;
+            if (comp) my_ixlo[j * blockDim.x] = 0.0;
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) src[q][j] = 0.0;
         }
@@ -232,18 +255,19 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             inj_from = inj < T ? slot_win[2 * inj] : NEVER;
         }
 
-        double *rb = ring + ((size_t)(phase * G + g) * W + rank) * P;   // by rank: fixed summation order
+        double *rb = ring + ((size_t)(phase * G + g) * W + warp) * P;   // summed by warp index: a fixed order
         if (na > 0) {
             double acc[NSRC][V];
 #pragma unroll
             for (int q = 0; q < NSRC; ++q)
 #pragma unroll
                 for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
-#define GCAMB_NA(n) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC>(tl0, ix, src, fa, fb, acc); break;
-            switch (na) {
-                GCAMB_NA(1) GCAMB_NA(2) GCAMB_NA(3) GCAMB_NA(4) GCAMB_NA(5)
-                GCAMB_NA(6) GCAMB_NA(7) GCAMB_NA(8) GCAMB_NA(9) GCAMB_NA(10)
-            }
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, blockDim.x, src, fa, fb, acc); break;
+#define GCAMB_BODIES(C) switch (na) { \
+                GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
+                GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) }
+            if (comp) { GCAMB_BODIES(true) } else { GCAMB_BODIES(false) }
+#undef GCAMB_BODIES
 #undef GCAMB_NA
             // cross-lane reduction into this warp's ring entry
             const double tot = warp_transpose_reduce<P>(&acc[0][0], scratch, lane);
@@ -337,8 +361,9 @@ static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &
     dim3 grid((unsigned)(prm.n_k * prm.n_batch), (unsigned)sh.n_split);
     const int W = sh.threads / 32;
     const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
-                        sizeof(double) * 2 * RING_G * W * NSRC * V + sizeof(int) * T * sh.threads +
-                        sizeof(int) * W * 2 * T;
+                        sizeof(double) * 2 * RING_G * W * NSRC * V +
+                        sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1) +
+                        sizeof(double) * T * sh.threads;
     // register budget: CTAs of <= 128 threads are compiled for GCAMB_MINB co-resident CTAs per SM
     auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB>
                                   : transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
@@ -383,6 +408,7 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
+    prm.n_comp = p->n_comp;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
     if (sh.n_split > 1) {
         const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;

@@ -19,7 +19,8 @@ GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI = 1, 2, 4
 _STATUS = {0: "GCAMB_OK", 1: "GCAMB_EINVAL", 2: "GCAMB_EGRID", 3: "GCAMB_EALLOC", 4: "GCAMB_ECUDA"}
 
 EXPORTS = (
-    "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_transfer",
+    "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
+    "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
     "gcamb_los_dfma_probe", "gcamb_los_last_error",
 )
@@ -48,6 +49,7 @@ def load_library() -> ctypes.CDLL:
                                           ctypes.c_uint32, _vp]
     lib.gcamb_los_plan_destroy.argtypes = [_vp]
     lib.gcamb_los_plan_info.argtypes = [_vp] + [ctypes.POINTER(_i32)] * 5 + [ctypes.POINTER(_i64)]
+    lib.gcamb_los_plan_launches.argtypes = [_vp, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]
     lib.gcamb_los_transfer.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_cls.argtypes = [_vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_transfer_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp]
@@ -112,7 +114,10 @@ class Plan:
         self.executed_terms = ex.value
         self.nominal_terms = self.n_l * self.n_k * self.n_tau
         # kernels of this library one transfer + one cls call launch (bench.py's gpu_launches)
-        self.launches_per_step = 2
+        nt, nc = _i32(), _i32()
+        _check(lib.gcamb_los_plan_launches(self._h, ctypes.byref(nt), ctypes.byref(nc)))
+        self.transfer_launches, self.cls_launches = nt.value, nc.value
+        self.launches_per_step = nt.value + nc.value
 
     def close(self) -> None:
         if getattr(self, "_h", None):

@@ -48,8 +48,11 @@ def cl_err(C_gpu, C_ref):
 
 def run_gpu(los, l_list, k, tau, tau0, S_T, S_E, S_P, P_R):
     plan = los.Plan(l_list, k, tau, tau0, with_phi=S_P is not None)
-    D = plan.gcamb_los_transfer(dev(S_T), dev(S_E), None if S_P is None else dev(S_P))
-    C = plan.gcamb_los_cls(D, dev(P_R))
+    # NaN pre-fill: an element the kernels fail to write cannot pass
+    D = torch.full((plan.n_src, plan.n_l, plan.n_k), float("nan"), dtype=torch.float64, device="cuda")
+    C = torch.full((plan.n_spec, plan.n_l), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer(dev(S_T), dev(S_E), None if S_P is None else dev(S_P), out=D)
+    plan.gcamb_los_cls(D, dev(P_R), out=C)
     torch.cuda.synchronize()
     out = D.cpu().numpy(), C.cpu().numpy(), plan
     return out
