@@ -38,6 +38,9 @@ UNIT = "terms/s"
 # FP64 roofline denominator: 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE transfer_kernel launch, from the committed
+# ncu --set full capture (profiles/r1_transfer_kernel.txt); only config 1 has been captured
+NCU_TRAFFIC_BYTES = {1: 130.072320e6 + 88.333824e6}
 
 
 def host_cores() -> int:
@@ -118,6 +121,21 @@ class ClockSampler:
         reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit]
         return {"sm_mhz": float(np.median(self.samples)), "sm_min_mhz": int(min(self.samples)),
                 "sm_max_mhz": self.sm_max, "reasons": reasons, "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------- multi-rank bookkeeping
+def max_over_ranks(times, dist, device):
+    """Element-wise maximum of a list of per-rank times over all ranks (the slowest rank decides)."""
+    import torch
+    tt = torch.tensor(list(times), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt.cpu()]
+
+
+def whole_job_rate(units_per_rank: float, world: int, t_max: float) -> float:
+    """Weak scaling over independent replicas: all ranks' units / the slowest rank's time."""
+    return units_per_rank * world / t_max
 
 
 # --------------------------------------------------------------------------- reference arm
@@ -281,10 +299,8 @@ def run_cuda(args) -> None:
     d2h = int(hCl.numel()) * 8
 
     # ---- max over ranks
-    tt = torch.tensor([t_step, t_e2e, float(np.mean(t_transfer)), float(np.mean(t_cls))], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_step, t_e2e, t_tr, t_cl = (float(v) for v in tt.cpu())
+    t_step, t_e2e, t_tr, t_cl = max_over_ranks(
+        [t_step, t_e2e, float(np.mean(t_transfer)), float(np.mean(t_cls))], dist, dev)
 
     nominal = plan.nominal_terms * B
     executed = plan.executed_terms * B
@@ -309,7 +325,7 @@ def run_cuda(args) -> None:
         return
 
     out = {
-        "metric": METRIC, "value": nominal * world / t_step, "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": whole_job_rate(nominal, world, t_step), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
@@ -327,7 +343,8 @@ def run_cuda(args) -> None:
         "gpu_launches": launches_per_step * args.steps,
         "roofline": {
             "bound": "alu", "kernel": "transfer_kernel", "achieved": achieved_tf, "peak": peak_tf,
-            "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+            "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_transfer_kernel.txt)",
             "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
                            f"dfma probe measured {probe_tf:.2f} TFLOP/s in this process",
             "algorithmic": f"{flop_per_term} flop per executed term x {executed} executed terms per launch",
