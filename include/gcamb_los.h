@@ -88,8 +88,10 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
 
 /*
  * Kernels of this library that one gcamb_los_transfer[_batched] call and one gcamb_los_cls[_batched]
- * call launch on this plan (any batch size; a cudaMemsetAsync of Delta precedes the transfer kernel
- * when the tau grid is split over several CTAs per k).  Either pointer may be NULL.
+ * call launch on this plan (any batch size).  The transfer is one launch, or two overlapping ones when
+ * only some rows (x_max = k (tau0 - tau_0) > 2^53 * 7.5e-13 = 6755) take the compensated recurrence
+ * coefficient; a cudaMemsetAsync of Delta precedes them when the
+ * tau grid is split over several CTAs per k.  Either pointer may be NULL.
  */
 gcamb_status gcamb_los_plan_launches(const gcamb_los_plan *plan, int32_t *transfer_kernels,
                                      int32_t *cls_kernels);

@@ -175,7 +175,7 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
 gcamb_status gcamb_los_plan_launches(const gcamb_los_plan *plan, int32_t *transfer_kernels, int32_t *cls_kernels)
 {
     if (!plan) { set_error("null plan"); return GCAMB_EINVAL; }
-    if (transfer_kernels) *transfer_kernels = 1;
+    if (transfer_kernels) *transfer_kernels = (plan->n_comp > 0) + (plan->n_comp < plan->n_k);
     if (cls_kernels) *cls_kernels = 1;
     return GCAMB_OK;
 }

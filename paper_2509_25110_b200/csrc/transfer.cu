@@ -32,7 +32,8 @@ struct TransferParams {
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
-    int n_comp;     // the first n_comp positions of korder (largest x) take the compensated coefficient
+    int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
+    int zero_fill;  // this launch also zeroes the skipped region of Delta (all rows of it)
 };
 
 constexpr unsigned FULL = 0xffffffffu;
@@ -109,7 +110,7 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
     }
 }
 
-template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS>
+template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
     static_assert(T >= 1 && T <= 10, "the NA dispatch below is written out for T <= 10");
@@ -128,8 +129,13 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) +
                                                  (((size_t)T * blockDim.x + W * 2 * T + 1) & ~(size_t)1)) + tid;
     const int bid = blockIdx.x;
-    const int krank = bid / p.n_batch, b = bid - krank * p.n_batch;   // krank: position in the cost order
-    const bool comp = krank < p.n_comp;   // CTA-uniform: this row takes the compensated coefficient
+    // The compensated rows run as their own small launch; the launch after it carries the
+    // programmatic-stream-serialization attribute and may start as soon as every CTA of this one has
+    // passed this point (the two launches write disjoint rows of Delta and never wait on each other).
+    asm volatile("griddepcontrol.launch_dependents;");
+    const int krel = bid / p.n_batch, b = bid - krel * p.n_batch;
+    const int krank = p.k_first + krel;   // position in the cost order
+    constexpr bool comp = COMP;           // this launch takes the compensated coefficient
     const int kidx = p.korder[krank];
     const int split = blockIdx.y;
     const int i_begin = split * p.split_len;
@@ -189,10 +195,10 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // every l, a prefix k < kz[tile of l] of the Delta row, so the CTAs share the rows among
     // themselves and zero them with coalesced stores (a CTA's own zero elements lie along l, 8 bytes
     // every n_k doubles).  With RED output the launcher zeroed the whole buffer instead.
-    if (p.n_split == 1) {
+    if (p.n_split == 1 && p.zero_fill) {
         if (p.kz) {
             const int n_rows = NSRC * p.n_l;
-            for (int r = krank; r < n_rows; r += gridDim.x / p.n_batch) {
+            for (int r = krel; r < n_rows; r += gridDim.x / p.n_batch) {
                 const int li = r % p.n_l;
                 const int nz = p.kz[(p.l_max - p.l_list[li]) / V];
                 double *dst = p.Delta + (delta_b + r) * p.n_k;
@@ -266,7 +272,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
                 GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) }
-            if (comp) { GCAMB_BODIES(true) } else { GCAMB_BODIES(false) }
+            GCAMB_BODIES(COMP)
 #undef GCAMB_BODIES
 #undef GCAMB_NA
             // cross-lane reduction into this warp's ring entry
@@ -324,6 +330,9 @@ constexpr int RING_G = GCAMB_G;   // tiles between CTA-wide flushes
 #ifndef GCAMB_MINB
 #define GCAMB_MINB 3
 #endif
+#ifndef GCAMB_MINB256
+#define GCAMB_MINB256 1
+#endif
 #ifndef GCAMB_V2
 #define GCAMB_V2 8          // l-tile for n_src = 2
 #endif
@@ -343,7 +352,11 @@ TransferShape choose_shape(int n_tau, int n_src)
         int best_pad = 0x7fffffff;
         // least padding wins; at equal padding the smaller CTA, i.e. more points per thread: the
         // cross-thread reduction costs one DADD per thread, tile row and source whatever T is
+#ifdef XP_THREADS_MIN
+        for (int threads = XP_THREADS_MIN; threads <= 256; threads <<= 1) {
+#else
         for (int threads = 32; threads <= 256; threads <<= 1) {
+#endif
             const int T = (len + threads - 1) / threads;
             if (T > t_max) continue;
             const int pad = T * threads - len;
@@ -355,39 +368,64 @@ TransferShape choose_shape(int n_tau, int n_src)
     return s;
 }
 
-template <int T, int V, int NSRC>
-static gcamb_status launch_impl(const TransferParams &prm, const TransferShape &sh, cudaStream_t stream)
+// One launch over positions [k_first, k_first + n_pos) of the cost order.
+template <int T, int V, int NSRC, bool COMP>
+static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int k_first, int n_pos,
+                                bool zero_fill, bool overlap_previous, cudaStream_t stream)
 {
-    dim3 grid((unsigned)(prm.n_k * prm.n_batch), (unsigned)sh.n_split);
+    if (n_pos <= 0) return GCAMB_OK;
+    prm.k_first = k_first;
+    prm.zero_fill = zero_fill;
     const int W = sh.threads / 32;
-    const size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
-                        sizeof(double) * 2 * RING_G * W * NSRC * V +
-                        sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1) +
-                        sizeof(double) * T * sh.threads;
+    size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
+                  sizeof(double) * 2 * RING_G * W * NSRC * V +
+                  sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1);
+    if (COMP) smem += sizeof(double) * T * sh.threads;
     // register budget: CTAs of <= 128 threads are compiled for GCAMB_MINB co-resident CTAs per SM
-    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB>
-                                  : transfer_kernel<T, V, NSRC, RING_G, 256, 1>;
+    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB, COMP>
+                                  : transfer_kernel<T, V, NSRC, RING_G, 256, GCAMB_MINB256, COMP>;
     if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, sh.threads, smem, stream>>>(prm);
-    GCAMB_CUDA(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(n_pos * prm.n_batch), (unsigned)sh.n_split);
+    cfg.blockDim = dim3((unsigned)sh.threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = overlap_previous ? 1 : 0;
+    GCAMB_CUDA(cudaLaunchKernelEx(&cfg, kern, prm));
     return GCAMB_OK;
 }
 
+// The first n_comp positions of the cost order (the largest k: x_max = k chi_0 above COMP_X_MIN)
+// run the compensated body in a launch of their own, issued first because they are the heaviest
+// rows; the plain launch follows, overlapped with it, and zero-fills.
+template <int T, int V, int NSRC>
+static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, cudaStream_t stream)
+{
+    const int n_plain = prm.n_k - n_comp;
+    gcamb_status st = launch_impl<T, V, NSRC, true>(prm, sh, 0, n_comp, n_plain == 0, false, stream);
+    if (st != GCAMB_OK) return st;
+    return launch_impl<T, V, NSRC, false>(prm, sh, n_comp, n_plain, true, n_comp > 0, stream);
+}
+
 template <int V, int NSRC>
-static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, cudaStream_t stream)
+static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, cudaStream_t stream)
 {
     switch (sh.T) {
-    case 1: return launch_impl<1, V, NSRC>(prm, sh, stream);
-    case 2: return launch_impl<2, V, NSRC>(prm, sh, stream);
-    case 3: return launch_impl<3, V, NSRC>(prm, sh, stream);
-    case 4: return launch_impl<4, V, NSRC>(prm, sh, stream);
-    case 5: return launch_impl<5, V, NSRC>(prm, sh, stream);
-    case 6: return launch_impl<6, V, NSRC>(prm, sh, stream);
-    case 7: return launch_impl<7, V, NSRC>(prm, sh, stream);
-    case 8: return launch_impl<8, V, NSRC>(prm, sh, stream);
-    case 9: return launch_impl<9, V, NSRC>(prm, sh, stream);
-    case 10: return launch_impl<10, V, NSRC>(prm, sh, stream);
+    case 1: return launch_pair<1, V, NSRC>(prm, sh, n_comp, stream);
+    case 2: return launch_pair<2, V, NSRC>(prm, sh, n_comp, stream);
+    case 3: return launch_pair<3, V, NSRC>(prm, sh, n_comp, stream);
+    case 4: return launch_pair<4, V, NSRC>(prm, sh, n_comp, stream);
+    case 5: return launch_pair<5, V, NSRC>(prm, sh, n_comp, stream);
+    case 6: return launch_pair<6, V, NSRC>(prm, sh, n_comp, stream);
+    case 7: return launch_pair<7, V, NSRC>(prm, sh, n_comp, stream);
+    case 8: return launch_pair<8, V, NSRC>(prm, sh, n_comp, stream);
+    case 9: return launch_pair<9, V, NSRC>(prm, sh, n_comp, stream);
+    case 10: return launch_pair<10, V, NSRC>(prm, sh, n_comp, stream);
     }
     set_error("no transfer kernel for T=%d", sh.T);
     return GCAMB_EINVAL;
@@ -408,14 +446,13 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
-    prm.n_comp = p->n_comp;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
     if (sh.n_split > 1) {
         const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
         GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
     }
-    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, stream);
-    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, stream);
+    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, p->n_comp, stream);
+    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, p->n_comp, stream);
     set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
     return GCAMB_EINVAL;
 }
