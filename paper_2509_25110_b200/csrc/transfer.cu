@@ -113,7 +113,7 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
 template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
-    static_assert(T >= 1 && T <= 10, "the NA dispatch below is written out for T <= 10");
+    static_assert(T >= 1 && T <= 12, "the NA dispatch below is written out for T <= 12");
     constexpr int P = NSRC * V;          // partial sums per thread and tile
     constexpr int NOUT = (G * P + MAXTHREADS - 1) / MAXTHREADS;   // flush outputs per thread (full CTA)
     // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] |
@@ -271,7 +271,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 #define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, blockDim.x, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
-                GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) }
+                GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) \
+                GCAMB_NA(11, C) GCAMB_NA(12, C) }
             GCAMB_BODIES(COMP)
 #undef GCAMB_BODIES
 #undef GCAMB_NA
@@ -345,7 +346,7 @@ TransferShape choose_shape(int n_tau, int n_src)
 {
     TransferShape s;
     s.V = n_src == 2 ? GCAMB_V2 : 8;
-    const int t_max = 10;
+    const int t_max = 12;
     s.n_split = 1;
     for (;;) {
         const int len = (n_tau + s.n_split - 1) / s.n_split;
@@ -381,8 +382,10 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
                   sizeof(double) * 2 * RING_G * W * NSRC * V +
                   sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1);
     if (COMP) smem += sizeof(double) * T * sh.threads;
-    // register budget: CTAs of <= 128 threads are compiled for GCAMB_MINB co-resident CTAs per SM
-    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, GCAMB_MINB, COMP>
+    // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
+    // are compiled for 3 co-resident CTAs per SM (168 registers) while that fits, else for 2
+    constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : GCAMB_MINB;
+    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP>
                                   : transfer_kernel<T, V, NSRC, RING_G, 256, GCAMB_MINB256, COMP>;
     if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -426,6 +429,8 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
     case 8: return launch_pair<8, V, NSRC>(prm, sh, n_comp, stream);
     case 9: return launch_pair<9, V, NSRC>(prm, sh, n_comp, stream);
     case 10: return launch_pair<10, V, NSRC>(prm, sh, n_comp, stream);
+    case 11: return launch_pair<11, V, NSRC>(prm, sh, n_comp, stream);
+    case 12: return launch_pair<12, V, NSRC>(prm, sh, n_comp, stream);
     }
     set_error("no transfer kernel for T=%d", sh.T);
     return GCAMB_EINVAL;
