@@ -119,7 +119,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] |
     // start tiles [T][threads] | slot first/last start tile [W][2T]
     extern __shared__ double2 smem2[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, W = blockDim.x >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, W = blockDim.x >> 5;
+    const int warp = __reduce_min_sync(0xffffffffu, tid >> 5);   // through a warp reduction: uniform register
     double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
     double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)warp * 32 * (P + 2);
     double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
@@ -187,7 +188,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     __syncwarp();
 
     // first tile of this CTA = start tile of its largest x
-    const int t_begin = p.tile[row + i_begin];
+    const int t_begin = __reduce_min_sync(FULL, p.tile[row + i_begin]);
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
 #define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
 
@@ -236,15 +237,18 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     prefetch_flush(t_begin);
 
     int na = 0;                               // started slots of this warp (warp-uniform)
-    int next_slot = slot_win[0];              // tile at which slot `na` starts
+    // warp-uniform bookkeeping is read through warp reductions (CREDUX), which puts it in uniform
+    // registers: branches on it need no convergence barrier and it takes no vector registers
+#define GCAMB_UNI(v) __reduce_min_sync(FULL, (v))
+    int next_slot = GCAMB_UNI(slot_win[0]);   // tile at which slot `na` starts
     int inj = 0;                              // first slot with points still to start (warp-uniform)
-    int inj_from = slot_win[0];               // its first start tile
+    int inj_from = next_slot;                 // its first start tile
     int phase = 0, g = 0, t_flush = t_begin;  // ring bookkeeping (CTA-uniform)
     double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);   // 2l+1 at the top of the tile
     for (int t = t_begin; t < p.n_tiles; ++t, tl0 -= 2.0 * V) {
         while (next_slot <= t) {
             ++na;
-            next_slot = na < T ? slot_win[2 * na] : NEVER;
+            next_slot = na < T ? GCAMB_UNI(slot_win[2 * na]) : NEVER;
         }
         // inject the plan's start pair (j_{lhi+1}, j_lhi) into points whose walk begins here;
         // skipped (warp-uniformly) on the tiles where no slot of this warp is inside its window
@@ -257,8 +261,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     fb[j] = st.y;
                 }
             }
-            while (inj < T && slot_win[2 * inj + 1] <= t) ++inj;
-            inj_from = inj < T ? slot_win[2 * inj] : NEVER;
+            while (inj < T && GCAMB_UNI(slot_win[2 * inj + 1]) <= t) ++inj;
+            inj_from = inj < T ? GCAMB_UNI(slot_win[2 * inj]) : NEVER;
         }
 
         double *rb = ring + ((size_t)(phase * G + g) * W + warp) * P;   // summed by warp index: a fixed order
