@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const int krel = bid / p.n_batch, b = bid - krel * p.n_batch;
     const int krank = p.k_first + krel;   // position in the cost order
     constexpr bool comp = COMP;           // this launch takes the compensated coefficient
-    const int kidx = p.korder[krank];
+    const int kidx = __reduce_min_sync(0xffffffffu, p.korder[krank]);   // uniform register, like the bookkeeping below
     const int split = blockIdx.y;
     const int i_begin = split * p.split_len;
     const int i_end = min(p.n_tau, i_begin + p.split_len);
@@ -219,10 +219,11 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 
     // flush bookkeeping: output `o` of this thread in a G-tile group is ring column
     // idx = tid + o*blockDim -> (tile gi, source q, row s); its l-index and Delta^E prefactor are
-    // fetched one group ahead so that the flush itself waits on no global load
+    // looked up at the flush (fetching them a group ahead costs registers across the tile loop and
+    // measured 0.8 % slower)
     int f_li[NOUT];
     double f_pref[NOUT];
-    auto prefetch_flush = [&](int t_first) {
+    auto flush_columns = [&](int t_first) {
 #pragma unroll
         for (int o = 0; o < NOUT; ++o) {
             const int idx = tid + o * (int)blockDim.x;
@@ -234,7 +235,6 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             f_pref[o] = (q == 1 && li >= 0) ? p.pref[li] : 1.0;
         }
     };
-    prefetch_flush(t_begin);
 
     int na = 0;                               // started slots of this warp (warp-uniform)
     // warp-uniform bookkeeping is read through warp reductions (CREDUX), which puts it in uniform
@@ -288,6 +288,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         }
 
         if (++g == G || t == p.n_tiles - 1) {
+            flush_columns(t_flush);
             // ---- flush: warps summed in fixed order, Delta^E prefactor, store
             __syncthreads();
             const double *fbuf = ring + (size_t)phase * G * W * P;
@@ -322,7 +323,6 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             phase ^= 1;
             g = 0;
             t_flush = t + 1;
-            prefetch_flush(t_flush);
         }
     }
 }
