@@ -131,11 +131,14 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
                                    void *cuda_stream);
 
 /*
- * End-to-end convenience with HOST buffers (the paper's "accelerator data region",
- * PAPER.md:133-136): H2D of the sources and P_R, transfer, cls, D2H of C_l (and of Delta when
- * h_Delta != NULL), then synchronises `cuda_stream`.  Device scratch is allocated inside the plan
- * on first use (sized for n_batch) and reused; not thread-safe per plan.  Host buffers should be
- * pinned for full copy bandwidth but need not be.
+ * End-to-end call with HOST buffers (the paper's "accelerator data region"):
+ * H2D of the sources and P_R, transfer, cls, D2H of C_l (and of Delta when h_Delta != NULL), then
+ * synchronises `cuda_stream`.  The sources are copied in four blocks of k rows (heaviest rows first)
+ * on a copy stream owned by the plan and each block's kernels start when it has landed, so the
+ * compute hides behind the H2D copy; results equal the device-resident path bit for bit.  Device
+ * scratch, streams and events are created inside the plan on first use (scratch sized for n_batch)
+ * and reused; NOT thread-safe per plan.  Host buffers should be pinned for full copy bandwidth
+ * (pageable memory works but serialises the copies).
  *   h_S_X HOST [n_batch][n_k][n_tau];  h_P_R HOST [n_batch][n_k];
  *   h_Cl  HOST [n_batch][n_spec][n_l]; h_Delta HOST [n_batch][n_src][n_l][n_k] or NULL.
  */

@@ -54,6 +54,11 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
+    if (p->h_streams_ready) {
+        cudaStreamDestroy(p->h_copy);
+        cudaEventDestroy(p->h_start);
+        for (int c = 0; c < 4; ++c) { cudaStreamDestroy(p->h_comp[c]); cudaEventDestroy(p->h_copied[c]); cudaEventDestroy(p->h_done[c]); }
+    }
     delete p;
 }
 
@@ -232,11 +237,54 @@ gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const
         p->host_batch_cap = n_batch;
     }
     const double *hS[3] = {h_S_T, h_S_E, h_S_phi};
-    for (int q = 0; q < p->n_src; ++q)
-        GCAMB_CUDA(cudaMemcpyAsync(p->d_hS[q], hS[q], sizeof(double) * nS * n_batch, cudaMemcpyHostToDevice, s));
     GCAMB_CUDA(cudaMemcpyAsync(p->d_hP, h_P_R, sizeof(double) * p->n_k * n_batch, cudaMemcpyHostToDevice, s));
-    st = launch_transfer(p, n_batch, p->d_hS[0], p->d_hS[1], p->d_hS[2], p->d_hDelta, s);
+
+    // The rows are processed heaviest first = k descending, so a range of cost-order positions is a
+    // contiguous block of k rows: the sources go up in NCH blocks on a copy stream and each block's
+    // kernels start on a stream of their own as soon as it has landed.  The first block is small
+    // (little to wait for, and its rows carry a third of the work), the last one is half the rows
+    // (light ones).  H2D of 8 n_src N_k N_tau bytes bounds the call; compute hides behind it.
+    constexpr int NCH = 4;
+    const bool pipelined = p->order_reversed && p->n_k >= 64;
+    if (pipelined && !p->h_streams_ready) {
+        GCAMB_CUDA(cudaStreamCreateWithFlags(&p->h_copy, cudaStreamNonBlocking));
+        GCAMB_CUDA(cudaEventCreateWithFlags(&p->h_start, cudaEventDisableTiming));
+        for (int c = 0; c < NCH; ++c) {
+            GCAMB_CUDA(cudaStreamCreateWithFlags(&p->h_comp[c], cudaStreamNonBlocking));
+            GCAMB_CUDA(cudaEventCreateWithFlags(&p->h_copied[c], cudaEventDisableTiming));
+            GCAMB_CUDA(cudaEventCreateWithFlags(&p->h_done[c], cudaEventDisableTiming));
+        }
+        p->h_streams_ready = 1;
+    }
+    st = launch_transfer_prepare(p, n_batch, p->d_hDelta, s);
     if (st != GCAMB_OK) return st;
+    if (!pipelined) {
+        for (int q = 0; q < p->n_src; ++q)
+            GCAMB_CUDA(cudaMemcpyAsync(p->d_hS[q], hS[q], sizeof(double) * nS * n_batch, cudaMemcpyHostToDevice, s));
+        st = launch_transfer_range(p, n_batch, p->d_hS[0], p->d_hS[1], p->d_hS[2], p->d_hDelta, 0, p->n_k, true, s);
+        if (st != GCAMB_OK) return st;
+    } else {
+        const int bound[NCH + 1] = {0, p->n_k / 16, p->n_k / 4, p->n_k / 2, p->n_k};
+        GCAMB_CUDA(cudaEventRecord(p->h_start, s));               // everything below follows the caller's stream
+        GCAMB_CUDA(cudaStreamWaitEvent(p->h_copy, p->h_start, 0));
+        const size_t pitch = sizeof(double) * nS;                  // one cosmology's [n_k][n_tau]
+        for (int c = 0; c < NCH; ++c) {
+            const int k_lo = p->n_k - bound[c + 1], rows = bound[c + 1] - bound[c];   // positions -> k rows
+            const size_t off = (size_t)k_lo * p->n_tau;
+            for (int q = 0; q < p->n_src; ++q)
+                GCAMB_CUDA(cudaMemcpy2DAsync(p->d_hS[q] + off, pitch, hS[q] + off, pitch,
+                                             sizeof(double) * (size_t)rows * p->n_tau, (size_t)n_batch,
+                                             cudaMemcpyHostToDevice, p->h_copy));
+            GCAMB_CUDA(cudaEventRecord(p->h_copied[c], p->h_copy));
+            GCAMB_CUDA(cudaStreamWaitEvent(p->h_comp[c], p->h_start, 0));
+            GCAMB_CUDA(cudaStreamWaitEvent(p->h_comp[c], p->h_copied[c], 0));
+            st = launch_transfer_range(p, n_batch, p->d_hS[0], p->d_hS[1], p->d_hS[2], p->d_hDelta,
+                                       bound[c], bound[c + 1], c == NCH - 1, p->h_comp[c]);
+            if (st != GCAMB_OK) return st;
+            GCAMB_CUDA(cudaEventRecord(p->h_done[c], p->h_comp[c]));
+            GCAMB_CUDA(cudaStreamWaitEvent(s, p->h_done[c], 0));
+        }
+    }
     st = launch_cls(p, n_batch, p->d_hDelta, p->d_hP, p->d_hCl, s);
     if (st != GCAMB_OK) return st;
     GCAMB_CUDA(cudaMemcpyAsync(h_Cl, p->d_hCl, sizeof(double) * nC * n_batch, cudaMemcpyDeviceToHost, s));

@@ -42,7 +42,12 @@ struct gcamb_los_plan {
     int32_t *d_l_list;   // [n_l] the l list
     int32_t *d_kz;       // [n_tiles] #k whose walk starts below tile t: Delta rows of tile t are 0 for k < kz[t]; NULL if not monotone
 
+    int32_t order_reversed;  // korder[r] == n_k - 1 - r: a range of positions is a contiguous range of k
+
     // scratch of gcamb_los_spectra_host (lazily allocated)
+    cudaStream_t h_copy, h_comp[4];
+    cudaEvent_t h_start, h_copied[4], h_done[4];
+    int32_t h_streams_ready;
     int32_t host_batch_cap;
     double *d_hS[3], *d_hP, *d_hDelta, *d_hCl;
 };
@@ -72,6 +77,12 @@ TransferShape choose_shape(int n_tau, int n_src);
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,
                              cudaStream_t stream);
+// the same in pieces, for the pipelined host entry point: `prepare` once, then any partition of the
+// cost-order positions [0, n_k) into ranges, exactly one of them (any) with zero_fill
+gcamb_status launch_transfer_prepare(const gcamb_los_plan *p, int n_batch, double *Delta, cudaStream_t stream);
+gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                                   const double *S_E, const double *S_phi, double *Delta,
+                                   int pos0, int pos1, bool zero_fill, cudaStream_t stream);
 
 // cls.cu
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,

@@ -146,6 +146,8 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     // ties (saturated rows) by k, so that the order is the k grid reversed whenever cost grows with k
     std::stable_sort(order.begin(), order.end(),
                      [&](int32_t a, int32_t b) { return cost[a] != cost[b] ? cost[a] > cost[b] : a > b; });
+    p->order_reversed = 1;
+    for (int r = 0; r < p->n_k; ++r) p->order_reversed = p->order_reversed && order[r] == p->n_k - 1 - r;
     GCAMB_CUDA(cudaMemcpyAsync(p->d_korder, order.data(), sizeof(int32_t) * p->n_k,
                                cudaMemcpyHostToDevice, stream));
     // rows whose largest x = k chi_max exceeds COMP_X_MIN run the compensated coefficient; they

@@ -20,6 +20,8 @@
 // every G tiles the CTA synchronises once, sums the warps in fixed order, applies the Delta^E
 // prefactor and stores.  The summation order is fixed by the launch shape alone, so results are
 // bit-reproducible and the batched call equals a loop of single calls.
+#include <algorithm>
+
 #include "los_internal.cuh"
 
 namespace gcamb {
@@ -407,34 +409,39 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     return GCAMB_OK;
 }
 
-// The first n_comp positions of the cost order (the largest k: x_max = k chi_0 above COMP_X_MIN)
-// run the compensated body in a launch of their own, issued first because they are the heaviest
-// rows; the plain launch follows, overlapped with it, and zero-fills.
+// Positions [pos0, pos1) of the cost order.  The first n_comp positions of the order (the largest
+// k: x_max = k chi_0 above COMP_X_MIN) run the compensated body in a launch of their own, issued
+// first because they are the heaviest rows; the plain launch follows, overlapped with it.
+// `zero_fill`: this range also zeroes the skipped region of Delta (for all rows).
 template <int T, int V, int NSRC>
-static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, cudaStream_t stream)
+static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
+                                bool zero_fill, cudaStream_t stream)
 {
-    const int n_plain = prm.n_k - n_comp;
-    gcamb_status st = launch_impl<T, V, NSRC, true>(prm, sh, 0, n_comp, n_plain == 0, false, stream);
+    const int c0 = pos0, c1 = std::min(pos1, n_comp);   // compensated part
+    const int q0 = std::max(pos0, n_comp), q1 = pos1;   // plain part
+    const bool has_plain = q1 > q0;
+    gcamb_status st = launch_impl<T, V, NSRC, true>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, stream);
     if (st != GCAMB_OK) return st;
-    return launch_impl<T, V, NSRC, false>(prm, sh, n_comp, n_plain, true, n_comp > 0, stream);
+    return launch_impl<T, V, NSRC, false>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, stream);
 }
 
 template <int V, int NSRC>
-static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, cudaStream_t stream)
+static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
+                             bool zero_fill, cudaStream_t stream)
 {
     switch (sh.T) {
-    case 1: return launch_pair<1, V, NSRC>(prm, sh, n_comp, stream);
-    case 2: return launch_pair<2, V, NSRC>(prm, sh, n_comp, stream);
-    case 3: return launch_pair<3, V, NSRC>(prm, sh, n_comp, stream);
-    case 4: return launch_pair<4, V, NSRC>(prm, sh, n_comp, stream);
-    case 5: return launch_pair<5, V, NSRC>(prm, sh, n_comp, stream);
-    case 6: return launch_pair<6, V, NSRC>(prm, sh, n_comp, stream);
-    case 7: return launch_pair<7, V, NSRC>(prm, sh, n_comp, stream);
-    case 8: return launch_pair<8, V, NSRC>(prm, sh, n_comp, stream);
-    case 9: return launch_pair<9, V, NSRC>(prm, sh, n_comp, stream);
-    case 10: return launch_pair<10, V, NSRC>(prm, sh, n_comp, stream);
-    case 11: return launch_pair<11, V, NSRC>(prm, sh, n_comp, stream);
-    case 12: return launch_pair<12, V, NSRC>(prm, sh, n_comp, stream);
+    case 1: return launch_pair<1, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 2: return launch_pair<2, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 3: return launch_pair<3, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 4: return launch_pair<4, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 5: return launch_pair<5, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 6: return launch_pair<6, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 7: return launch_pair<7, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 8: return launch_pair<8, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 9: return launch_pair<9, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 10: return launch_pair<10, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 11: return launch_pair<11, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+    case 12: return launch_pair<12, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
     }
     set_error("no transfer kernel for T=%d", sh.T);
     return GCAMB_EINVAL;
@@ -443,6 +450,24 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,
                              cudaStream_t stream)
+{
+    gcamb_status st = launch_transfer_prepare(p, n_batch, Delta, stream);
+    if (st != GCAMB_OK) return st;
+    return launch_transfer_range(p, n_batch, S_T, S_E, S_phi, Delta, 0, p->n_k, true, stream);
+}
+
+gcamb_status launch_transfer_prepare(const gcamb_los_plan *p, int n_batch, double *Delta, cudaStream_t stream)
+{
+    if (p->shape.n_split > 1) {   // RED output: the tau splits add into a zeroed Delta
+        const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
+        GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
+    }
+    return GCAMB_OK;
+}
+
+gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                                   const double *S_E, const double *S_phi, double *Delta,
+                                   int pos0, int pos1, bool zero_fill, cudaStream_t stream)
 {
     const TransferShape &sh = p->shape;
     TransferParams prm;
@@ -456,12 +481,8 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
-    if (sh.n_split > 1) {
-        const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
-        GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
-    }
-    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, p->n_comp, stream);
-    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, p->n_comp, stream);
+    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
+    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
     set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
     return GCAMB_EINVAL;
 }

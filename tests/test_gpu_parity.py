@@ -155,6 +155,27 @@ def test_host_buffer_entry_point_matches_device_path(los):
     assert np.array_equal(Cl[0], C.cpu().numpy()) and np.array_equal(Dl[0], D.cpu().numpy())
 
 
+@pytest.mark.parametrize("with_phi", [False, True])
+def test_pipelined_host_entry_point_batched(los, with_phi):
+    """n_k >= 64: the sources go up in four blocks of k rows that overlap the kernels of the blocks
+    before them; results must equal the device-resident path bit for bit, for a batch too."""
+    cfg = synth.Config(9, "mini-pipe", 2, 400, 150, 1e-4, 0.25, 100, 60, with_phi, n_batch=3)
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, with_phi=with_phi)
+    S = [synth.sources(cfg, c) for c in range(cfg.n_batch)]
+    hS = [np.stack([s[q] for s in S]) if S[0][q] is not None else None for q in range(3)]
+    hP = np.stack([synth.primordial_power(cfg, c) for c in range(cfg.n_batch)])
+    D = plan.gcamb_los_transfer_batched(dev(hS[0]), dev(hS[1]), None if hS[2] is None else dev(hS[2]))
+    C = plan.gcamb_los_cls_batched(D, dev(hP))
+    Cl = np.full((cfg.n_batch, plan.n_spec, cfg.n_l), np.nan)
+    Dl = np.full((cfg.n_batch, plan.n_src, cfg.n_l, cfg.n_k), np.nan)
+    for _ in range(2):          # the second call reuses the plan's streams and scratch
+        plan.gcamb_los_spectra_host(hS[0], hS[1], hS[2], hP, Cl, Dl)
+        assert np.array_equal(Cl, C.cpu().numpy()) and np.array_equal(Dl, D.cpu().numpy())
+    D_ref = oracle.transfer(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, S[1][0], S[1][1], S[1][2], real="f80")
+    assert delta_err(Dl[1], D_ref) <= TOL_DELTA
+    plan.close()
+
+
 def test_errors_cross_the_abi_as_status_codes(los):
     cfg = synth.CONFIGS[0]
     with pytest.raises(los.GcambError) as e:
