@@ -38,9 +38,10 @@ UNIT = "terms/s"
 # FP64 roofline denominator: 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE transfer_kernel launch, from the committed
-# ncu --set full capture (profiles/r1_transfer_kernel.txt); only config 1 has been captured
-NCU_TRAFFIC_BYTES = {1: 130.072320e6 + 88.333824e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE gcamb_los_transfer call (its plain launch plus
+# its small compensated-rows launch), from the committed ncu --set full capture
+# (profiles/r1_transfer_kernel_plain.txt, r1_transfer_kernel_compensated.txt); only config 1 was captured
+NCU_TRAFFIC_BYTES = {1: (127.435264e6 + 84.549120e6) + (2.526208e6 + 0.0)}
 
 
 def host_cores() -> int:
@@ -344,7 +345,7 @@ def run_cuda(args) -> None:
         "roofline": {
             "bound": "alu", "kernel": "transfer_kernel", "achieved": achieved_tf, "peak": peak_tf,
             "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_transfer_kernel.txt)",
+            "traffic_unit": "bytes per transfer call (ncu dram read+write, profiles/r1_transfer_kernel_*.txt)",
             "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
                            f"dfma probe measured {probe_tf:.2f} TFLOP/s in this process",
             "algorithmic": f"{flop_per_term} flop per executed term x {executed} executed terms per launch",
