@@ -33,7 +33,8 @@ def build_extension(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = f"{LIB}.{os.getpid()}.tmp"
-    cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+    debug = ["-DGCAMB_DEBUG"] if os.environ.get("GCAMB_DEBUG") == "1" else []   # device asserts on every index
+    cmd = [nvcc, *NVCC_FLAGS, *debug, *(["-Xptxas", "-v"] if verbose else []),
            *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)

@@ -22,7 +22,18 @@
 // bit-reproducible and the batched call equals a loop of single calls.
 #include <algorithm>
 
+#include <cassert>
+
 #include "los_internal.cuh"
+
+// compute-sanitizer is not available on the target pool: a build with -DGCAMB_DEBUG (GCAMB_DEBUG=1
+// python -m paper_2509_25110_b200.build --force) checks every global and ring index of the transfer
+// kernel with device asserts instead; the GPU tests are run once against that build per change.
+#ifdef GCAMB_DEBUG
+#define GCAMB_ASSERT(c) assert(c)
+#else
+#define GCAMB_ASSERT(c) ((void)0)
+#endif
 
 namespace gcamb {
 
@@ -161,6 +172,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         int tp = NEVER;
         if (i < i_end) {
             const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + i;
+            GCAMB_ASSERT(kidx >= 0 && kidx < p.n_k && b < p.n_batch && i >= 0 && i < p.n_tau && krank < p.n_k);
             const double x = __dmul_rn(kval, p.chi[i]);
             const double inv = 1.0 / x;
             const double w = p.w[i];
@@ -205,6 +217,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                 const int li = r % p.n_l;
                 const int nz = p.kz[(p.l_max - p.l_list[li]) / V];
                 double *dst = p.Delta + (delta_b + r) * p.n_k;
+                GCAMB_ASSERT(nz >= 0 && nz <= p.n_k && r < n_rows && li < p.n_l);
                 for (int j = tid; j < nz; j += blockDim.x) dst[j] = 0.0;
             }
         } else {
@@ -268,6 +281,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         }
 
         double *rb = ring + ((size_t)(phase * G + g) * W + warp) * P;   // summed by warp index: a fixed order
+        GCAMB_ASSERT(g >= 0 && g < G && (phase == 0 || phase == 1) && warp < W && t >= 0 && na <= T);
         if (na > 0) {
             double acc[NSRC][V];
 #pragma unroll
@@ -304,6 +318,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
                     sum *= f_pref[o];
                     double *dst = p.Delta + DIDX(q, li);
+                    GCAMB_ASSERT(q < NSRC && li < p.n_l && gi < G && (size_t)(dst - p.Delta) < (size_t)p.n_batch * NSRC * p.n_l * p.n_k);
                     if (p.n_split == 1) *dst = sum;
                     else atomicAdd(dst, sum);
                 }

@@ -112,6 +112,48 @@ def test_edge_shapes(los, case):
     assert e_auto <= TOL_CL and e_te <= TOL_CL
 
 
+def test_batched_tau_split_with_phi(los):
+    """n_tau above one CTA's slots: two CTAs share a k and add into the zeroed Delta (RED path);
+    batched, three sources, sparse l list; still equal to the single calls bit for bit."""
+    rng = np.random.default_rng(11)
+    n_k, n_tau, B = 7, 3300, 3
+    tau = np.sort(rng.uniform(100.0, 13900.0, n_tau))
+    k = np.geomspace(1e-4, 0.05, n_k)
+    l_list = np.array([2, 3, 9, 10, 11, 64, 65, 200, 399, 640], dtype=np.int32)
+    S = rng.standard_normal((3, B, n_k, n_tau))
+    P = rng.uniform(1e-9, 3e-9, (B, n_k))
+    plan = los.Plan(l_list, k, tau, 14000.0, with_phi=True)
+    Db = torch.full((B, 3, l_list.size, n_k), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer_batched(dev(S[0]), dev(S[1]), dev(S[2]), out=Db)
+    Cb = plan.gcamb_los_cls_batched(Db, dev(P))
+    for c in range(B):
+        D1 = plan.gcamb_los_transfer(dev(S[0, c]), dev(S[1, c]), dev(S[2, c]))
+        assert torch.equal(D1, Db[c])
+        D_ref = oracle.transfer(l_list, k, tau, 14000.0, S[0, c], S[1, c], S[2, c], real="f80")
+        C_ref = oracle.cls(k, D_ref, P[c], real="f80")
+        assert delta_err(Db[c].cpu().numpy(), D_ref) <= TOL_DELTA
+        e_auto, e_te = cl_err(Cb[c].cpu().numpy(), C_ref)
+        assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
+def test_rows_that_never_start_and_rows_above_the_compensation_threshold(los):
+    """l range far above x for the small k (their Delta rows are all zero, the CTA walks nothing)
+    together with k rows whose x_max exceeds 6755 (compensated coefficient launch)."""
+    tau = np.concatenate([np.linspace(200.0, 400.0, 70), np.geomspace(420.0, 13999.0, 50)])
+    k = np.concatenate([np.geomspace(1e-5, 1e-3, 6), np.linspace(0.3, 0.62, 9)])
+    l_list = np.arange(1500, 1640, dtype=np.int32)
+    rng = np.random.default_rng(5)
+    S_T, S_E = rng.standard_normal((2, k.size, tau.size))
+    P = np.full(k.size, 2e-9)
+    D, C, plan = run_gpu(los, l_list, k, tau, 14000.0, S_T, S_E, None, P)
+    assert plan.transfer_launches == 2
+    assert np.all(D[:, :, :6] == 0.0)                      # x <= 14 there, l >= 1500
+    D_ref = oracle.transfer(l_list, k, tau, 14000.0, S_T, S_E, real="f80")
+    assert delta_err(D, D_ref) <= TOL_DELTA
+    plan.close()
+
+
 def test_single_tau_source_is_the_kernel(los):
     """P3 on the GPU: S = delta_{i,i*}/w_{i*} gives Delta_l(k) = j_l(k chi*) (values: oracle column)."""
     tau = np.array([100.0, 280.0, 700.0, 13000.0])
