@@ -218,6 +218,33 @@ def test_pipelined_host_entry_point_batched(los, with_phi):
     plan.close()
 
 
+def test_transfer_and_cls_capture_into_a_cuda_graph(los):
+    """The calls only enqueue work on the given stream (no allocation, no synchronisation), so a
+    step can be captured once and replayed (emulator loops)."""
+    cfg = synth.CONFIGS[0]
+    S_T, S_E, _ = synth.sources(cfg)
+    plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0)
+    d_T, d_E, d_P = dev(S_T), dev(S_E), dev(synth.primordial_power(cfg))
+    D = torch.empty(2, cfg.n_l, cfg.n_k, dtype=torch.float64, device="cuda")
+    C = torch.empty(3, cfg.n_l, dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer(d_T, d_E, out=D)
+    plan.gcamb_los_cls(D, d_P, out=C)
+    torch.cuda.synchronize()
+    D0, C0 = D.clone(), C.clone()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            plan.gcamb_los_transfer(d_T, d_E, out=D)
+            plan.gcamb_los_cls(D, d_P, out=C)
+    for _ in range(2):
+        D.fill_(float("nan"))
+        C.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(D, D0) and torch.equal(C, C0)
+    plan.close()
+
+
 def test_errors_cross_the_abi_as_status_codes(los):
     cfg = synth.CONFIGS[0]
     with pytest.raises(los.GcambError) as e:
