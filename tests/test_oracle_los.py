@@ -9,6 +9,7 @@ closed forms for int j_l^2 x^-p dln x: 1/(2l(l+1)) (p=0, the Sachs-Wolfe plateau
 4 pi ln(k_max/k_min); Cauchy-Schwarz.
 """
 import math
+import os
 
 import mpmath as mp
 import numpy as np
@@ -211,3 +212,48 @@ def test_bad_arguments():
         oracle.transfer(cfg.l_list(), [-1.0, 2.0], cfg.tau(), cfg.tau0, S, S)
     with pytest.raises(ValueError):
         oracle.transfer(cfg.l_list(), [1.0, 2.0], cfg.tau(), cfg.tau()[-1], S, S)
+
+
+def _survey_golden():
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "config0_survey.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                rows.append(line.split())
+    return rows
+
+
+def test_generator_spot_values_of_survey_a5():
+    """grids and noisy sources of config 0 (libm-dependent at the ulp level: 1e-13)."""
+    cfg = synth.CONFIGS[0]
+    arrays = {"k": cfg.k(), "tau": cfg.tau()}
+    arrays["S_T"], arrays["S_E"], _ = synth.sources(cfg)
+    n = 0
+    for row in _survey_golden():
+        if row[0] in arrays:
+            idx = tuple(int(v) for v in row[1:-1])
+            assert arrays[row[0]][idx] == pytest.approx(float(row[-1]), rel=1e-13)
+            n += 1
+    assert n == 7
+
+
+@pytest.mark.parametrize("real", REALS)
+def test_p9_config0_spectra_against_the_surveys_independent_prototype(real):
+    """C_l of config 0 from an implementation written before and without this
+    oracle (numpy long double, all-downward recurrence).  Pins the whole pipeline -- grids, weights,
+    Bessel columns, Delta^E prefactor and 1/x^2, ln k weights, 4 pi -- at config 0 to the 12 printed
+    digits (TE relative to sqrt(TE^2 + TT EE), reading R13: it crosses zero between l = 100 and 150)."""
+    cfg = synth.CONFIGS[0]
+    S_T, S_E, _ = synth.sources(cfg)
+    D = oracle.transfer(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, S_T, S_E, real=real)
+    C = oracle.cls(cfg.k(), D, synth.primordial_power(cfg), real=real)
+    n = 0
+    for row in _survey_golden():
+        if row[0] == "cl":
+            a = int(row[1]) - cfg.l_min
+            tt, ee, te = (float(v) for v in row[2:])
+            assert C[0, a] == pytest.approx(tt, rel=2e-12)
+            assert C[1, a] == pytest.approx(ee, rel=2e-12)
+            assert abs(C[2, a] - te) <= 2e-12 * np.sqrt(te * te + tt * ee)
+            n += 1
+    assert n == 7
