@@ -261,3 +261,63 @@ def test_errors_cross_the_abi_as_status_codes(los):
     with pytest.raises(los.GcambError) as e:
         plan.gcamb_los_transfer(z, z, z)                                # phi source without the mask bit
     assert e.value.status == 1
+
+
+# --------------------------------------------------------------------------- seeded random shapes
+@pytest.mark.parametrize("seed", range(32))
+def test_random_small_shapes(los, seed):
+    """Seeded random grids and l lists around the kernel's shape boundaries (one warp to several
+    CTAs per k, dense and sparse l lists, l ranges far above or below x, with and without phi,
+    with and without a batch), element by element against the long-double oracle.
+
+    Unlike BASELINE.json's configs (k_max tau0 ~ 2 l_max) these l ranges may lie entirely above
+    x + 18 x^(1/3) for every k, where Delta_l consists of nothing but terms the skip rule drops
+    (R16: |j_l(x)| < 1e-30 may be skipped); the bar therefore carries the rule's own allowance,
+    1e-30 sum_i |w_i S_X(k,tau_i)| (times the Delta^E factor), next to 1e-10 max_k |Delta_l|."""
+    rng = np.random.default_rng(1000 + seed)
+    n_tau = int(rng.choice([2, 3, 31, 32, 33, 64, 127, 128, 129, 300, 641, 1281, 1537, 2600]))
+    n_k = int(rng.integers(2, 12))
+    with_phi = bool(rng.integers(0, 2))
+    B = int(rng.choice([1, 1, 2, 3]))
+    tau0 = 14000.0
+    tau = np.sort(rng.uniform(10.0, 13999.0, n_tau))
+    tau = np.unique(tau)
+    n_tau = tau.size
+    k_hi = float(rng.choice([1e-3, 0.02, 0.2, 0.61]))
+    k = np.sort(k_hi * rng.uniform(1e-3, 1.0, n_k))
+    k = np.unique(k)
+    n_k = k.size
+    l_lo = int(rng.choice([2, 2, 17, 300, 1200]))
+    l_hi = l_lo + int(rng.choice([0, 1, 7, 8, 9, 63, 200, 700]))
+    l_all = np.arange(l_lo, l_hi + 1)
+    if rng.integers(0, 2) and l_all.size > 3:
+        l_all = np.sort(rng.choice(l_all, size=max(2, l_all.size // int(rng.integers(2, 9))), replace=False))
+    l_list = l_all.astype(np.int32)
+    S = rng.standard_normal((3, B, n_k, n_tau)) * np.exp(rng.uniform(-20, 5, (3, B, n_k, 1)))
+    P = rng.uniform(1e-9, 3e-9, (B, n_k))
+    plan = los.Plan(l_list, k, tau, tau0, with_phi=with_phi)
+    n_src = 3 if with_phi else 2
+    D = torch.full((B, n_src, l_list.size, n_k), float("nan"), dtype=torch.float64, device="cuda")
+    C = torch.full((B, n_src + 1, l_list.size), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer_batched(dev(S[0]), dev(S[1]), dev(S[2]) if with_phi else None, out=D)
+    plan.gcamb_los_cls_batched(D, dev(P), out=C)
+    torch.cuda.synchronize()
+    D, C = D.cpu().numpy(), C.cpu().numpy()
+    for c in range(B):
+        D_ref = oracle.transfer(l_list, k, tau, tau0, S[0, c], S[1, c], S[2, c] if with_phi else None, real="f80")
+        C_ref = oracle.cls(k, D_ref, P[c], real="f80")
+        w = oracle.trapz_weights(tau)
+        x = k[:, None] * (tau0 - tau)[None, :]
+        pref = np.sqrt((l_list + 2.0) * (l_list + 1.0) * l_list * (l_list - 1.0))
+        skip = [np.sum(np.abs(w * S[0, c]), axis=1)[None, :] * np.ones((l_list.size, 1)),
+                np.sum(np.abs(w * S[1, c]) / x ** 2, axis=1)[None, :] * pref[:, None]]
+        if with_phi:
+            skip.append(np.sum(np.abs(w * S[2, c]), axis=1)[None, :] * np.ones((l_list.size, 1)))
+        bound = TOL_DELTA * np.max(np.abs(D_ref), axis=-1, keepdims=True) + 1e-30 * np.stack(skip)
+        assert np.all(np.abs(D[c] - D_ref) <= bound), (seed, n_tau, n_k, with_phi, B, l_lo, l_hi)
+        big = np.max(np.abs(D_ref), axis=-1) > 1e-12 * np.max(np.abs(D_ref))      # rows far above the skip level
+        ok = (C_ref[0] * C_ref[1] > 0) & big[0] & big[1]
+        if ok.any():
+            e_auto, e_te = cl_err(C[c][:, ok], C_ref[:, ok])
+            assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
