@@ -5,17 +5,23 @@
 from __future__ import annotations
 
 import os
+import shutil
 import subprocess
 import sys
+import tempfile
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgcamb_los.so")
-SOURCES = ["api.cu", "plan.cu", "transfer.cu", "cls.cu"]
+# (source, extra flags, object tag): transfer.cu is compiled once per (sparse, n_src) entry, in parallel
+UNITS = [("api.cu", [], "api"), ("plan.cu", [], "plan"), ("cls.cu", [], "cls")] + [
+    ("transfer.cu", [f"-DGCAMB_TU_SPARSE={sp}", f"-DGCAMB_TU_NSRC={ns}"], f"transfer_s{sp}n{ns}")
+    for sp in (0, 1) for ns in (2, 3)]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared",
+    "--fmad=true", "-Xcompiler", "-fPIC", "-cudart", "shared",
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 
@@ -32,11 +38,23 @@ def build_extension(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = f"{LIB}.{os.getpid()}.tmp"
     debug = ["-DGCAMB_DEBUG"] if os.environ.get("GCAMB_DEBUG") == "1" else []   # device asserts on every index
-    cmd = [nvcc, *NVCC_FLAGS, *debug, *(["-Xptxas", "-v"] if verbose else []),
-           *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
-    subprocess.run(cmd, check=True)
+    objdir = tempfile.mkdtemp(prefix="gcamb_build_")
+    try:
+        def compile_unit(unit):
+            src, flags, tag = unit
+            obj = os.path.join(objdir, tag + ".o")
+            cmd = [nvcc, *NVCC_FLAGS, *debug, *flags, *(["-Xptxas", "-v"] if verbose else []),
+                   "-c", os.path.join(CSRC, src), "-o", obj]
+            subprocess.run(cmd, check=True)
+            return obj
+        with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 1)) as pool:
+            objs = list(pool.map(compile_unit, UNITS))
+        tmp = f"{LIB}.{os.getpid()}.tmp"
+        subprocess.run([nvcc, "-shared", "-cudart", "shared", "-gencode", "arch=compute_100a,code=sm_100a",
+                        *objs, "-o", tmp], check=True)
+    finally:
+        shutil.rmtree(objdir, ignore_errors=True)
     os.replace(tmp, LIB)
     return LIB
 

@@ -51,7 +51,7 @@ static void free_plan(gcamb_los_plan *p)
     if (!p) return;
     cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
     cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile);
-    cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz);
+    cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     if (p->h_streams_ready) {
@@ -136,6 +136,16 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     cudaError_t e = cudaGetDevice(&p->device);
     if (e == cudaSuccess) e = upload(&p->d_l_index, l_index, stream);
     if (e == cudaSuccess) e = upload(&p->d_l_list, std::vector<int32_t>(l_list, l_list + n_l), stream);
+    {   // sparse l lists: which tiles hold a listed l (NULL table = all of them)
+        std::vector<uint32_t> mask((p->n_tiles + 31) / 32, 0u);
+        for (int i = 0; i < n_l; ++i) {
+            const int t = (p->l_max - l_list[i]) / p->shape.V;
+            mask[t >> 5] |= 1u << (t & 31);
+        }
+        int listed = 0;
+        for (int t = 0; t < p->n_tiles; ++t) listed += (mask[t >> 5] >> (t & 31)) & 1u;
+        if (listed < p->n_tiles && e == cudaSuccess) e = upload(&p->d_tile_mask, mask, stream);
+    }
     if (e == cudaSuccess) e = upload(&p->d_k, vk, stream);
     if (e == cudaSuccess) e = upload(&p->d_chi, chi, stream);
     if (e == cudaSuccess) e = upload(&p->d_w, w, stream);

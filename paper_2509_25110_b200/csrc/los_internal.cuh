@@ -40,6 +40,7 @@ struct gcamb_los_plan {
     int32_t *d_tile;     // [n_k][n_tau] first l-tile of the point
     int32_t *d_korder;   // [n_k] k indices, heaviest first
     int32_t *d_l_list;   // [n_l] the l list
+    uint32_t *d_tile_mask;   // [ceil(n_tiles/32)] bit t%32 of word t/32: tile t holds a listed l; NULL when every tile does
     int32_t *d_kz;       // [n_tiles] #k whose walk starts below tile t: Delta rows of tile t are 0 for k < kz[t]; NULL if not monotone
 
     int32_t order_reversed;  // korder[r] == n_k - 1 - r: a range of positions is a contiguous range of k

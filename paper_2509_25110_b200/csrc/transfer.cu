@@ -43,6 +43,7 @@ struct TransferParams {
     const double *k, *chi, *w, *pref;
     const double2 *start;
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
+    const uint32_t *tile_mask;   // [ceil(n_tiles/32)] bit = the tile holds an l of the list (sparse lists only)
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
     int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
@@ -123,7 +124,33 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
     }
 }
 
-template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP>
+// A tile none of whose l is in the l list (sparse lists, R21: CAMB's default l sampling computes
+// about every 50th l): only the recurrence walks it, 2 FP64 instructions per term, no accumulators,
+// no reduction.  The NA chains are interleaved (l outer, slot inner): without the accumulates a
+// single slot's 8-step DFMA chain would be latency-bound.
+template <int NA, int T, int V, bool COMP>
+__device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T], const double *ixlo, int stride,
+                                               double (&fa)[T], double (&fb)[T])
+{
+    double e[NA];
+    if (COMP) {
+#pragma unroll
+        for (int j = 0; j < NA; ++j) e[j] = tl0 * ixlo[j * stride];
+    }
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+        const double tl = tl0 - 2.0 * s;
+#pragma unroll
+        for (int j = 0; j < NA; ++j) {
+            const double c = COMP ? fma(tl, ix[j], e[j]) : tl * ix[j];
+            const double fn = fma(c, fb[j], -fa[j]);
+            fa[j] = fb[j];
+            fb[j] = fn;
+        }
+    }
+}
+
+template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
     static_assert(T >= 1 && T <= 12, "the NA dispatch below is written out for T <= 12");
@@ -259,6 +286,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     int inj = 0;                              // first slot with points still to start (warp-uniform)
     int inj_from = next_slot;                 // its first start tile
     int phase = 0, g = 0, t_flush = t_begin;  // ring bookkeeping (CTA-uniform)
+    unsigned mask_word = 0;                   // SPARSE: bit (t & 31) of tile_mask[t >> 5] = tile t holds a listed l
+    bool g_any = false;                       // SPARSE: some tile of the current group does
     double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);   // 2l+1 at the top of the tile
     for (int t = t_begin; t < p.n_tiles; ++t, tl0 -= 2.0 * V) {
         while (next_slot <= t) {
@@ -280,9 +309,22 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             inj_from = inj < T ? GCAMB_UNI(slot_win[2 * inj]) : NEVER;
         }
 
+        bool acc_on = true;   // this tile holds an l of the list (always, unless SPARSE)
+        if constexpr (SPARSE) {
+            if ((t & 31) == 0 || t == t_begin) mask_word = __reduce_min_sync(FULL, p.tile_mask[t >> 5]);
+            acc_on = (mask_word >> (t & 31)) & 1u;
+            g_any |= acc_on;
+        }
         double *rb = ring + ((size_t)(phase * G + g) * W + warp) * P;   // summed by warp index: a fixed order
         GCAMB_ASSERT(g >= 0 && g < G && (phase == 0 || phase == 1) && warp < W && t >= 0 && na <= T);
-        if (na > 0) {
+        if (SPARSE && !acc_on) {
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C>(tl0, ix, my_ixlo, blockDim.x, fa, fb); break;
+            switch (na) {
+                GCAMB_NA(1, COMP) GCAMB_NA(2, COMP) GCAMB_NA(3, COMP) GCAMB_NA(4, COMP) GCAMB_NA(5, COMP) GCAMB_NA(6, COMP)
+                GCAMB_NA(7, COMP) GCAMB_NA(8, COMP) GCAMB_NA(9, COMP) GCAMB_NA(10, COMP) GCAMB_NA(11, COMP) GCAMB_NA(12, COMP)
+            }
+#undef GCAMB_NA
+        } else if (na > 0) {
             double acc[NSRC][V];
 #pragma unroll
             for (int q = 0; q < NSRC; ++q)
@@ -304,6 +346,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         }
 
         if (++g == G || t == p.n_tiles - 1) {
+            if (SPARSE && !g_any) {   // no listed l in this group (the same for every warp): nothing to flush
+                g = 0;
+                t_flush = t + 1;
+                continue;
+            }
+            g_any = false;
             flush_columns(t_flush);
             // ---- flush: warps summed in fixed order, Delta^E prefactor, store
             __syncthreads();
@@ -363,6 +411,7 @@ constexpr int RING_G = GCAMB_G;   // tiles between CTA-wide flushes
 // to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA advances at the pace of
 // its slowest warp, so warp counts such as 5 leave one pipe with twice the work of the others
 // (measured: profiles/README.md).  T is then the smallest slot count that covers the tau range.
+#if !defined(GCAMB_TU_SPARSE) || (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
 TransferShape choose_shape(int n_tau, int n_src)
 {
     TransferShape s;
@@ -389,9 +438,10 @@ TransferShape choose_shape(int n_tau, int n_src)
     }
     return s;
 }
+#endif
 
 // One launch over positions [k_first, k_first + n_pos) of the cost order.
-template <int T, int V, int NSRC, bool COMP>
+template <int T, int V, int NSRC, bool COMP, bool SPARSE>
 static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int k_first, int n_pos,
                                 bool zero_fill, bool overlap_previous, cudaStream_t stream)
 {
@@ -406,8 +456,8 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
     // are compiled for 3 co-resident CTAs per SM (168 registers) while that fits, else for 2
     constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : GCAMB_MINB;
-    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP>
-                                  : transfer_kernel<T, V, NSRC, RING_G, 256, GCAMB_MINB256, COMP>;
+    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE>
+                                  : transfer_kernel<T, V, NSRC, RING_G, 256, GCAMB_MINB256, COMP, SPARSE>;
     if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     cudaLaunchConfig_t cfg = {};
@@ -428,40 +478,68 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
 // k: x_max = k chi_0 above COMP_X_MIN) run the compensated body in a launch of their own, issued
 // first because they are the heaviest rows; the plain launch follows, overlapped with it.
 // `zero_fill`: this range also zeroes the skipped region of Delta (for all rows).
-template <int T, int V, int NSRC>
+// SPARSE: the kernels that skip the accumulation on tiles without a listed l (sparse l lists).
+template <int T, int V, int NSRC, bool SPARSE>
 static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
                                 bool zero_fill, cudaStream_t stream)
 {
     const int c0 = pos0, c1 = std::min(pos1, n_comp);   // compensated part
     const int q0 = std::max(pos0, n_comp), q1 = pos1;   // plain part
     const bool has_plain = q1 > q0;
-    gcamb_status st = launch_impl<T, V, NSRC, true>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, stream);
+    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, stream);
     if (st != GCAMB_OK) return st;
-    return launch_impl<T, V, NSRC, false>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, stream);
+    return launch_impl<T, V, NSRC, false, SPARSE>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, stream);
 }
 
-template <int V, int NSRC>
+template <int V, int NSRC, bool SPARSE>
 static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
                              bool zero_fill, cudaStream_t stream)
 {
     switch (sh.T) {
-    case 1: return launch_pair<1, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 2: return launch_pair<2, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 3: return launch_pair<3, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 4: return launch_pair<4, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 5: return launch_pair<5, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 6: return launch_pair<6, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 7: return launch_pair<7, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 8: return launch_pair<8, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 9: return launch_pair<9, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 10: return launch_pair<10, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 11: return launch_pair<11, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
-    case 12: return launch_pair<12, V, NSRC>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+#define GCAMB_T(t) case t: return launch_pair<t, V, NSRC, SPARSE>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+        GCAMB_T(1) GCAMB_T(2) GCAMB_T(3) GCAMB_T(4) GCAMB_T(5) GCAMB_T(6)
+        GCAMB_T(7) GCAMB_T(8) GCAMB_T(9) GCAMB_T(10) GCAMB_T(11) GCAMB_T(12)
+#undef GCAMB_T
     }
     set_error("no transfer kernel for T=%d", sh.T);
     return GCAMB_EINVAL;
 }
 
+// The kernel instantiations (12 T x 2 coefficient forms x 2 CTA sizes per entry) dominate the build,
+// so build.py compiles this file four times, once per entry below (-DGCAMB_TU_SPARSE=s
+// -DGCAMB_TU_NSRC=n), in parallel; the host-side functions live in the (0, 2) unit.  Without the
+// macros everything is one translation unit.
+#ifdef GCAMB_TU_SPARSE
+#define GCAMB_TU_HAS(sp, ns) ((sp) == GCAMB_TU_SPARSE && (ns) == GCAMB_TU_NSRC)
+#define GCAMB_TU_PRIMARY (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
+#else
+#define GCAMB_TU_HAS(sp, ns) 1
+#define GCAMB_TU_PRIMARY 1
+#endif
+#define GCAMB_ENTRY(name, NS, SP)                                                                             \
+    gcamb_status name(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,     \
+                      bool zero_fill, cudaStream_t stream)                                                    \
+    {                                                                                                         \
+        return launch_T<(NS) == 2 ? GCAMB_V2 : 8, NS, SP>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);    \
+    }
+gcamb_status launch_range_dense_2(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
+gcamb_status launch_range_dense_3(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
+gcamb_status launch_range_sparse_2(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
+gcamb_status launch_range_sparse_3(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
+#if GCAMB_TU_HAS(0, 2)
+GCAMB_ENTRY(launch_range_dense_2, 2, false)
+#endif
+#if GCAMB_TU_HAS(0, 3)
+GCAMB_ENTRY(launch_range_dense_3, 3, false)
+#endif
+#if GCAMB_TU_HAS(1, 2)
+GCAMB_ENTRY(launch_range_sparse_2, 2, true)
+#endif
+#if GCAMB_TU_HAS(1, 3)
+GCAMB_ENTRY(launch_range_sparse_3, 3, true)
+#endif
+
+#if GCAMB_TU_PRIMARY
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,
                              cudaStream_t stream)
@@ -490,16 +568,20 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.Delta = Delta;
     prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref;
     prm.start = p->d_start; prm.tile = p->d_tile; prm.korder = p->d_korder; prm.l_index = p->d_l_index;
-    prm.l_list = p->d_l_list; prm.kz = p->d_kz;
+    prm.l_list = p->d_l_list; prm.kz = p->d_kz; prm.tile_mask = p->d_tile_mask;
     prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l;
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
-    if (p->n_src == 2 && sh.V == GCAMB_V2) return launch_T<GCAMB_V2, 2>(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
-    if (p->n_src == 3 && sh.V == 8) return launch_T<8, 3>(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
+    const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
+    if (p->n_src == 2 && sh.V == GCAMB_V2)
+        return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
+    if (p->n_src == 3 && sh.V == 8)
+        return (sparse ? launch_range_sparse_3 : launch_range_dense_3)(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
     set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
     return GCAMB_EINVAL;
 }
+#endif   // GCAMB_TU_PRIMARY
 
 }  // namespace gcamb

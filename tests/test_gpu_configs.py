@@ -188,3 +188,24 @@ def test_config4_extreme(los):
     assert e_auto <= TOL_CL and e_te <= TOL_CL
     assert np.all(D_s[D_ref == 0.0] == 0.0)
     plan_s.close()
+
+
+def test_config1_sparse_l_list_equals_the_dense_rows(los):
+    """R21 at config-1 size: an l list sampled like CAMB's default (every l at low l, every 50th
+    above; `l_sample_boost`).  Tiles without a listed l are walked by the
+    recurrence only; the listed rows must equal those of the all-l run bit for bit."""
+    cfg = synth.CONFIGS[1]
+    l_sparse = np.unique(np.concatenate([np.arange(2, 40), np.arange(40, 200, 10),
+                                         np.arange(200, 2501, 50), [2499, 2500]])).astype(np.int32)
+    S_T, S_E, _ = synth.sources(cfg)
+    d_T, d_E = dev(S_T), dev(S_E)
+    dense = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0)
+    sparse = los.Plan(l_sparse, cfg.k(), cfg.tau(), cfg.tau0)
+    D_dense = dense.gcamb_los_transfer(d_T, d_E)
+    D_sparse = nan_like(2, l_sparse.size, cfg.n_k)
+    sparse.gcamb_los_transfer(d_T, d_E, out=D_sparse)
+    torch.cuda.synchronize()
+    rows = torch.from_numpy(l_sparse.astype(np.int64) - cfg.l_min).cuda()
+    assert torch.equal(D_sparse, D_dense[:, rows, :])
+    dense.close()
+    sparse.close()
