@@ -67,6 +67,10 @@ static gcamb_status check_call(const gcamb_los_plan *p, int n_batch, const doubl
 {
     if (!p || !S_T || !S_E || !out) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
     if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    if ((long long)p->n_k * n_batch > 0x7fffffffLL) {   // one CTA per (k, cosmology) along grid.x
+        set_error("n_k * n_batch must be below 2^31");
+        return GCAMB_EINVAL;
+    }
     if ((p->n_src == 3) != (S_phi != nullptr)) {
         set_error("S_phi must be non-NULL exactly when the plan has GCAMB_SRC_PHI");
         return GCAMB_EINVAL;
