@@ -50,7 +50,7 @@ static void free_plan(gcamb_los_plan *p)
 {
     if (!p) return;
     cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
-    cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile);
+    cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile); cudaFree(p->d_inv);
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
@@ -158,6 +158,7 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     const size_t npt = (size_t)n_k * n_tau;
     if (e == cudaSuccess) e = cudaMalloc(&p->d_start, sizeof(double2) * npt);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_tile, sizeof(int32_t) * npt);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_inv, sizeof(double) * npt);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_korder, sizeof(int32_t) * n_k);
     // the uploads read pageable vectors that die with this scope
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);

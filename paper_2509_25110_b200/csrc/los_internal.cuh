@@ -38,6 +38,7 @@ struct gcamb_los_plan {
     double *d_pref;      // [n_l]   sqrt((l+2)(l+1)l(l-1))
     double2 *d_start;    // [n_k][n_tau] (j_{lhi+1}(x), j_{lhi}(x)), lhi = l_max - V*tile
     int32_t *d_tile;     // [n_k][n_tau] first l-tile of the point
+    double *d_inv;       // [n_k][n_tau] 1/x
     int32_t *d_korder;   // [n_k] k indices, heaviest first
     int32_t *d_l_list;   // [n_l] the l list
     uint32_t *d_tile_mask;   // [ceil(n_tiles/32)] bit t%32 of word t/32: tile t holds a listed l; NULL when every tile does

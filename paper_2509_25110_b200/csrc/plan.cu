@@ -40,7 +40,8 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
                                                            const double *__restrict__ chi, int n_tau,
                                                            int l_max, int V,
                                                            double2 *__restrict__ start,
-                                                           int32_t *__restrict__ tile)
+                                                           int32_t *__restrict__ tile,
+                                                           double *__restrict__ inv_x)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y;
@@ -83,6 +84,7 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
     const size_t idx = (size_t)j * n_tau + i;
     start[idx] = out;
     tile[idx] = t;
+    inv_x[idx] = inv;   // 1/x, correctly rounded: the transfer kernel's coefficient base
 }
 
 // per-k work: walked = sum_i (lhi_i - l_min + 1)+, executed = sum_i (min(L(x_i), l_max) - l_min + 1)+
@@ -122,7 +124,7 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     const int V = p->shape.V;
     dim3 grid((p->n_tau + 127) / 128, p->n_k);
     start_values_kernel<<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V,
-                                                  p->d_start, p->d_tile);
+                                                  p->d_start, p->d_tile, p->d_inv);
     GCAMB_CUDA(cudaGetLastError());
 
     long long *d_cost = nullptr;

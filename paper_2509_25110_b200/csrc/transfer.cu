@@ -40,7 +40,7 @@ namespace gcamb {
 struct TransferParams {
     const double *S[3];
     double *Delta;
-    const double *k, *chi, *w, *pref;
+    const double *k, *chi, *w, *pref, *inv_x;
     const double2 *start;
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     const uint32_t *tile_mask;   // [ceil(n_tiles/32)] bit = the tile holds an l of the list (sparse lists only)
@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + i;
             GCAMB_ASSERT(kidx >= 0 && kidx < p.n_k && b < p.n_batch && i >= 0 && i < p.n_tau && krank < p.n_k);
             const double x = __dmul_rn(kval, p.chi[i]);
-            const double inv = 1.0 / x;
+            const double inv = p.inv_x[row + i];   // 1/x from the plan: no division in the per-call path
             const double w = p.w[i];
             ix[j] = inv;
             if (comp) {   // 1/x = inv + inv_lo,  inv_lo = -inv * (inv x - 1), the residual taken exactly by the fma
@@ -566,7 +566,7 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     TransferParams prm;
     prm.S[0] = S_T; prm.S[1] = S_E; prm.S[2] = S_phi;
     prm.Delta = Delta;
-    prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref;
+    prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref; prm.inv_x = p->d_inv;
     prm.start = p->d_start; prm.tile = p->d_tile; prm.korder = p->d_korder; prm.l_index = p->d_l_index;
     prm.l_list = p->d_l_list; prm.kz = p->d_kz; prm.tile_mask = p->d_tile_mask;
     prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l;
