@@ -91,6 +91,36 @@ __device__ __forceinline__ double warp_transpose_reduce(const double *vals, doub
     return sum;
 }
 
+// ---- ring of partial sums between the warps of a CTA, and its shared-memory mbarriers.
+// The walk is cut into groups of G tiles; group n lives in ring stage n % RD.  A warp that has
+// written its partial sums of group n arrives on full[stage] and then flushes its share of group
+// n - LAG, whose full[] barrier has normally completed long before; having read it, it arrives on
+// empty[stage], which a warp awaits before it writes group n + RD - LAG ... into that stage again.
+// So a warp only ever waits when it is more than a group ahead of the slowest warp of its CTA,
+// instead of at every group as with __syncthreads (10 % of the warp time was barrier wait: the
+// warps sit on different sub-partitions and have different numbers of started slots).
+// Measured: RD = 3, LAG = 1 best (-2 %); more stages or more lag are slower.
+constexpr int RD = 3;    // ring stages
+constexpr int LAG = 1;   // a group is flushed this many groups after it was written (<= RD - 2)
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, int parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+
 // a2 + a3 for one l-tile and the first NA slots of this thread: NA independent recurrence chains.
 // Slots are taken one after the other (j outer, l inner): the V recurrence steps of a slot form
 // one dependent DFMA chain (8 cycles each, measured), which the 4-5 FP64 instructions of a step
@@ -164,11 +194,15 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
     double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)warp * 32 * (P + 2);
     double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
-    int *my_tile = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + tid;   // [j * blockDim]
-    int *slot_win = reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) + (size_t)T * blockDim.x + warp * 2 * T;
+    int *my_tile = reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) + tid;   // [j * blockDim]
+    int *slot_win = reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) + (size_t)T * blockDim.x + warp * 2 * T;
     // compensated rows only: residuals of the rounded reciprocals [T][threads], after the (8-byte aligned) int tables
-    double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)2 * G * W * P) +
+    double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) +
                                                  (((size_t)T * blockDim.x + W * 2 * T + 1) & ~(size_t)1)) + tid;
+    const uint32_t bar_full = (uint32_t)__cvta_generic_to_shared(ring + (size_t)RD * G * W * P);
+    const uint32_t bar_empty = bar_full + 8 * RD;
+    if (tid == 0) for (int d = 0; d < 2 * RD; ++d) mbar_init(bar_full + 8 * d, W);
+    __syncthreads();
     const int bid = blockIdx.x;
     // The compensated rows run as their own small launch; the launch after it carries the
     // programmatic-stream-serialization attribute and may start as soon as every CTA of this one has
@@ -278,6 +312,50 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         }
     };
 
+    const int n_walk = p.n_tiles - t_begin;
+    // flush of group m: the warps' entries summed in fixed order (by warp index), Delta^E prefactor,
+    // store.  `has`: some tile of the group holds a listed l (always, unless SPARSE).
+    auto flush_group = [&](int m, bool has) {
+        const int stage = m % RD;
+        const int t_first = t_begin + m * G;
+        const int gcount = min(G, n_walk - m * G);
+        if (has) {
+            flush_columns(t_first);
+            mbar_wait(bar_full + 8 * stage, (m / RD) & 1);
+            const double *fbuf = ring + (size_t)stage * G * W * P;
+#pragma unroll
+            for (int o = 0; o < NOUT; ++o) {
+                const int idx = tid + o * (int)blockDim.x;
+                const int li = f_li[o];
+                if (idx < gcount * P && li >= 0) {
+                    const int gi = idx / P, r = idx - gi * P, q = r / V;
+                    double sum = 0.0;
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    sum *= f_pref[o];
+                    double *dst = p.Delta + DIDX(q, li);
+                    if (p.n_split == 1) *dst = sum;
+                    else atomicAdd(dst, sum);
+                }
+            }
+            // CTAs smaller than the one NOUT was sized for: the remaining columns
+            for (int idx = tid + NOUT * (int)blockDim.x; idx < gcount * P; idx += blockDim.x) {
+                const int gi = idx / P, r = idx - gi * P, q = r / V, s = r - q * V;
+                const int l = p.l_max - (t_first + gi) * V - s;
+                const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
+                if (li >= 0) {
+                    double sum = 0.0;
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    if (q == 1) sum *= p.pref[li];
+                    double *dst = p.Delta + DIDX(q, li);
+                    if (p.n_split == 1) *dst = sum;
+                    else atomicAdd(dst, sum);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * stage);
+    };
+
     int na = 0;                               // started slots of this warp (warp-uniform)
     // warp-uniform bookkeeping is read through warp reductions (CREDUX), which puts it in uniform
     // registers: branches on it need no convergence barrier and it takes no vector registers
@@ -285,11 +363,19 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     int next_slot = GCAMB_UNI(slot_win[0]);   // tile at which slot `na` starts
     int inj = 0;                              // first slot with points still to start (warp-uniform)
     int inj_from = next_slot;                 // its first start tile
-    int phase = 0, g = 0, t_flush = t_begin;  // ring bookkeeping (CTA-uniform)
+    unsigned any_hist = 0;                    // bit i: group n - i holds a listed l (SPARSE; else every group)
     unsigned mask_word = 0;                   // SPARSE: bit (t & 31) of tile_mask[t >> 5] = tile t holds a listed l
-    bool g_any = false;                       // SPARSE: some tile of the current group does
     double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);   // 2l+1 at the top of the tile
-    for (int t = t_begin; t < p.n_tiles; ++t, tl0 -= 2.0 * V) {
+    const int n_groups = (n_walk + G - 1) / G;
+    int t = t_begin;
+    // group n is walked in iteration n and flushed in iteration n + LAG (one call site for the flush)
+    for (int n = 0; n < n_groups + LAG; ++n) {
+      bool g_any = false;                     // some tile of this group holds a listed l
+      if (n < n_groups) {
+        g_any = !SPARSE;
+        if (n >= RD) mbar_wait(bar_empty + 8 * (n % RD), ((n / RD) - 1) & 1);
+        const int gcount = min(G, n_walk - n * G);
+        for (int g = 0; g < gcount; ++g, ++t, tl0 -= 2.0 * V) {
         while (next_slot <= t) {
             ++na;
             next_slot = na < T ? GCAMB_UNI(slot_win[2 * na]) : NEVER;
@@ -315,8 +401,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             acc_on = (mask_word >> (t & 31)) & 1u;
             g_any |= acc_on;
         }
-        double *rb = ring + ((size_t)(phase * G + g) * W + warp) * P;   // summed by warp index: a fixed order
-        GCAMB_ASSERT(g >= 0 && g < G && (phase == 0 || phase == 1) && warp < W && t >= 0 && na <= T);
+        double *rb = ring + ((size_t)((n % RD) * G + g) * W + warp) * P;   // summed by warp index: a fixed order
+        GCAMB_ASSERT(g >= 0 && g < G && warp < W && t >= 0 && na <= T && n * G + g == t - t_begin);
         if (SPARSE && !acc_on) {
 #define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C>(tl0, ix, my_ixlo, blockDim.x, fa, fb); break;
             switch (na) {
@@ -345,50 +431,12 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             for (int idx = lane; idx < P; idx += 32) rb[idx] = 0.0;
         }
 
-        if (++g == G || t == p.n_tiles - 1) {
-            if (SPARSE && !g_any) {   // no listed l in this group (the same for every warp): nothing to flush
-                g = 0;
-                t_flush = t + 1;
-                continue;
-            }
-            g_any = false;
-            flush_columns(t_flush);
-            // ---- flush: warps summed in fixed order, Delta^E prefactor, store
-            __syncthreads();
-            const double *fbuf = ring + (size_t)phase * G * W * P;
-#pragma unroll
-            for (int o = 0; o < NOUT; ++o) {
-                const int idx = tid + o * (int)blockDim.x;
-                const int li = f_li[o];
-                if (idx < g * P && li >= 0) {
-                    const int gi = idx / P, r = idx - gi * P, q = r / V;
-                    double sum = 0.0;
-                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
-                    sum *= f_pref[o];
-                    double *dst = p.Delta + DIDX(q, li);
-                    GCAMB_ASSERT(q < NSRC && li < p.n_l && gi < G && (size_t)(dst - p.Delta) < (size_t)p.n_batch * NSRC * p.n_l * p.n_k);
-                    if (p.n_split == 1) *dst = sum;
-                    else atomicAdd(dst, sum);
-                }
-            }
-            // CTAs smaller than the one NOUT was sized for: the remaining columns, unprefetched
-            for (int idx = tid + NOUT * (int)blockDim.x; idx < g * P; idx += blockDim.x) {
-                const int gi = idx / P, r = idx - gi * P, q = r / V, s = r - q * V;
-                const int l = p.l_max - (t_flush + gi) * V - s;
-                const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
-                if (li >= 0) {
-                    double sum = 0.0;
-                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
-                    if (q == 1) sum *= p.pref[li];
-                    double *dst = p.Delta + DIDX(q, li);
-                    if (p.n_split == 1) *dst = sum;
-                    else atomicAdd(dst, sum);
-                }
-            }
-            phase ^= 1;
-            g = 0;
-            t_flush = t + 1;
-        }
+        }   // tiles of the group
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_full + 8 * (n % RD));
+      }
+      any_hist = (any_hist << 1) | (unsigned)g_any;
+      if (n >= LAG) flush_group(n - LAG, (any_hist >> LAG) & 1u);
     }
 }
 
@@ -450,7 +498,7 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     prm.zero_fill = zero_fill;
     const int W = sh.threads / 32;
     size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
-                  sizeof(double) * 2 * RING_G * W * NSRC * V +
+                  sizeof(double) * (RD * RING_G * W * NSRC * V + 2 * RD) +
                   sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1);
     if (COMP) smem += sizeof(double) * T * sh.threads;
     // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
