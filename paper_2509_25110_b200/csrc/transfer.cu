@@ -78,8 +78,10 @@ __device__ __forceinline__ double warp_transpose_reduce(const double *vals, doub
     double s0 = 0.0, s1 = 0.0;
     if (col < P) {
         const double *base = scratch + (size_t)grp * ROWS * RS + col;
+        s0 = base[0];          // not 0.0 + base[0]: the compiler keeps that add (it turns -0 into +0)
+        s1 = base[RS];
 #pragma unroll
-        for (int r = 0; r < ROWS; r += 2) {
+        for (int r = 2; r < ROWS; r += 2) {
             s0 += base[r * RS];
             s1 += base[(r + 1) * RS];
         }
