@@ -45,6 +45,7 @@ struct TransferParams {
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     const uint32_t *tile_mask;   // [ceil(n_tiles/32)] bit = the tile holds an l of the list (sparse lists only)
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
+    int order_reversed;   // korder[r] == n_k - 1 - r
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
     int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
     int zero_fill;  // this launch also zeroes the skipped region of Delta (all rows of it)
@@ -213,7 +214,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const int krel = bid / p.n_batch, b = bid - krel * p.n_batch;
     const int krank = p.k_first + krel;   // position in the cost order
     constexpr bool comp = COMP;           // this launch takes the compensated coefficient
-    const int kidx = __reduce_min_sync(0xffffffffu, p.korder[krank]);   // uniform register, like the bookkeeping below
+    // the cost order is the k grid reversed whenever cost grows with k: no table look-up then
+    const int kidx = p.order_reversed ? p.n_k - 1 - krank : __reduce_min_sync(0xffffffffu, p.korder[krank]);   // uniform register, like the bookkeeping below
     const int split = blockIdx.y;
     const int i_begin = split * p.split_len;
     const int i_end = min(p.n_tau, i_begin + p.split_len);
@@ -227,45 +229,60 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // result must not depend on where it sits in the launch) to give
     // every warp the same mix of heavy and light ranks; the lanes of a warp slot are 32 consecutive
     // tau and start within a tile or two of each other (lockstep waste ~1%).
+    // zero-prefix lengths of the (at most two, normally) Delta rows this CTA zero-fills: looked up here
+    // so that the look-ups travel with the prologue loads instead of adding their own round trips
+    const int zf_rows = NSRC * p.n_l, zf_step = gridDim.x / p.n_batch;
+    const bool zf = p.n_split == 1 && p.zero_fill && p.kz != nullptr;
+    int zf_nz[2] = {0, 0};
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        const int r = krel + u * zf_step;
+        if (zf && r < zf_rows) {
+            const int li = r % p.n_l;
+            zf_nz[u] = p.kz[(p.l_max - (p.l_contig ? p.l_min + li : p.l_list[li])) / V];
+        }
+    }
+    // first tile of this CTA = start tile of its largest x (loaded here, with the rest of the prologue)
+    const int t_begin_load = p.tile[row + i_begin];
     double fa[T], fb[T], ix[T], src[NSRC][T];
+    // Branch-free: slots past the end of the tau range read a clamped (valid) index and are masked
+    // afterwards, so that the ~6 T loads of a thread are all in flight together instead of one
+    // slot's round trip to L2/HBM after the other (the prologue was 11 % of the warp time).
+    int tp[T];
 #pragma unroll
     for (int j = 0; j < T; ++j) {
         const int i = i_begin + j * (int)blockDim.x + ((warp + j) % W) * 32 + lane;
+        const bool valid = i < i_end;
+        const int ic = valid ? i : i_end - 1;
+        const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + ic;
+        GCAMB_ASSERT(kidx >= 0 && kidx < p.n_k && b < p.n_batch && ic >= 0 && ic < p.n_tau && krank < p.n_k);
+        const double inv = p.inv_x[row + ic];   // 1/x from the plan: no division in the per-call path
+        const double w = valid ? p.w[ic] : 0.0;
         fa[j] = fb[j] = 0.0;
-        int tp = NEVER;
-        if (i < i_end) {
-            const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + i;
-            GCAMB_ASSERT(kidx >= 0 && kidx < p.n_k && b < p.n_batch && i >= 0 && i < p.n_tau && krank < p.n_k);
-            const double x = __dmul_rn(kval, p.chi[i]);
-            const double inv = p.inv_x[row + i];   // 1/x from the plan: no division in the per-call path
-            const double w = p.w[i];
-            ix[j] = inv;
-            if (comp) {   // 1/x = inv + inv_lo,  inv_lo = -inv * (inv x - 1), the residual taken exactly by the fma
-                const double res = fma(inv, x, -1.0);
-                my_ixlo[j * blockDim.x] = -inv * res;
-            }
-            tp = p.tile[row + i];
-            my_start[j * blockDim.x] = p.start[row + i];
-            src[0][j] = w * p.S[0][sx];
-            src[1][j] = w * p.S[1][sx] * (inv * inv);
-            if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
-        } else {
-            ix[j] = 0.0;
-            if (comp) my_ixlo[j * blockDim.x] = 0.0;
-#pragma unroll
-            for (int q = 0; q < NSRC; ++q) src[q][j] = 0.0;
+        ix[j] = valid ? inv : 0.0;
+        if (comp) {   // 1/x = inv + inv_lo,  inv_lo = -inv * (inv x - 1), the residual taken exactly by the fma
+            const double x = __dmul_rn(kval, p.chi[ic]);
+            const double res = fma(inv, x, -1.0);
+            my_ixlo[j * blockDim.x] = valid ? -inv * res : 0.0;
         }
-        my_tile[j * blockDim.x] = tp;
+        tp[j] = valid ? p.tile[row + ic] : NEVER;
+        my_start[j * blockDim.x] = p.start[row + ic];   // never injected when the slot is masked (tile NEVER)
+        src[0][j] = w * p.S[0][sx];
+        src[1][j] = w * p.S[1][sx] * (inv * inv);
+        if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
+        my_tile[j * blockDim.x] = tp[j];
+    }
+#pragma unroll
+    for (int j = 0; j < T; ++j) {
         // x falls with tau: within a warp every point of slot j starts no later than any point of
         // slot j+1, so the start windows [first, last] of the slots are ordered
-        const int first = __reduce_min_sync(FULL, tp);
-        const int last = __reduce_max_sync(FULL, tp == NEVER ? -1 : tp);
+        const int first = __reduce_min_sync(FULL, tp[j]);
+        const int last = __reduce_max_sync(FULL, tp[j] == NEVER ? -1 : tp[j]);
         if (lane == 0) { slot_win[2 * j] = first; slot_win[2 * j + 1] = last; }
     }
     __syncwarp();
 
-    // first tile of this CTA = start tile of its largest x
-    const int t_begin = __reduce_min_sync(FULL, p.tile[row + i_begin]);
+    const int t_begin = __reduce_min_sync(FULL, t_begin_load);
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
 #define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
 
@@ -275,12 +292,13 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // every n_k doubles).  With RED output the launcher zeroed the whole buffer instead.
     if (p.n_split == 1 && p.zero_fill) {
         if (p.kz) {
-            const int n_rows = NSRC * p.n_l;
-            for (int r = krel; r < n_rows; r += gridDim.x / p.n_batch) {
+            int u = 0;
+            for (int r = krel; r < zf_rows; r += zf_step, ++u) {
                 const int li = r % p.n_l;
-                const int nz = p.kz[(p.l_max - p.l_list[li]) / V];
+                const int nz = u < 2 ? zf_nz[u < 1 ? 0 : 1]
+                                     : p.kz[(p.l_max - (p.l_contig ? p.l_min + li : p.l_list[li])) / V];
                 double *dst = p.Delta + (delta_b + r) * p.n_k;
-                GCAMB_ASSERT(nz >= 0 && nz <= p.n_k && r < n_rows && li < p.n_l);
+                GCAMB_ASSERT(nz >= 0 && nz <= p.n_k && r < zf_rows && li < p.n_l);
                 for (int j = tid; j < nz; j += blockDim.x) dst[j] = 0.0;
             }
         } else {
@@ -623,6 +641,7 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
     prm.n_batch = n_batch; prm.n_split = sh.n_split;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
+    prm.order_reversed = p->order_reversed;
     prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
     if (p->n_src == 2 && sh.V == GCAMB_V2)
