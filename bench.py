@@ -41,7 +41,7 @@ L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE gcamb_los_transfer call (its plain launch plus
 # its small compensated-rows launch), from the committed ncu --set full capture
 # (profiles/r1_transfer_kernel_plain.txt, r1_transfer_kernel_compensated.txt); only config 1 was captured
-NCU_TRAFFIC_BYTES = {1: (155.764992e6 + 90.693120e6) + (3.063040e6 + 0.0)}
+NCU_TRAFFIC_BYTES = {1: (155.694336e6 + 91.366656e6) + (3.065088e6 + 0.0)}
 
 
 def host_cores() -> int:

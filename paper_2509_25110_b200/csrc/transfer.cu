@@ -119,7 +119,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, int parity)
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n"   // suspend-time hint: the warp sleeps in hardware instead of spinning through issue slots
         "@!p bra WAIT_%=;\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
