@@ -58,7 +58,7 @@ constexpr int NEVER = 0x7fffffff;
 // [q][s]); lane c < P returns the sum over the 32 lanes of partial c, in a fixed order.
 // Transposed through a per-warp shared-memory scratch [32][P+2] (the +2 keeps the 16-byte stores
 // of a quarter-warp on distinct banks).  With C = the power of two >= P, the warp splits into
-// 32/C lane groups; group g sums rows g*C .. g*C+C-1 of column lane%C in two interleaved chains
+// 32/C lane groups; group g sums rows g*C .. g*C+C-1 of column lane%C in four interleaved chains
 // (DADD latency, not throughput, bounds a single chain), then the groups are combined by xor
 // shuffles: P/2 STS.128 + C LDS.64 + (C + log2(32/C)) DADD per lane, against ~9 issue slots per
 // partial for a shuffle butterfly -- on sm_100a an FP64 instruction holds its sub-partition's
@@ -76,18 +76,22 @@ __device__ __forceinline__ double warp_transpose_reduce(const double *vals, doub
     for (int i = 0; i < P / 2; ++i) row[i] = make_double2(vals[2 * i], vals[2 * i + 1]);
     __syncwarp();
     const int col = lane & (C - 1), grp = lane / C;
-    double s0 = 0.0, s1 = 0.0;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
     if (col < P) {
         const double *base = scratch + (size_t)grp * ROWS * RS + col;
         s0 = base[0];          // not 0.0 + base[0]: the compiler keeps that add (it turns -0 into +0)
         s1 = base[RS];
+        s2 = base[2 * RS];
+        s3 = base[3 * RS];
 #pragma unroll
-        for (int r = 2; r < ROWS; r += 2) {
+        for (int r = 4; r < ROWS; r += 4) {
             s0 += base[r * RS];
             s1 += base[(r + 1) * RS];
+            s2 += base[(r + 2) * RS];
+            s3 += base[(r + 3) * RS];
         }
     }
-    double sum = s0 + s1;
+    double sum = (s0 + s1) + (s2 + s3);
 #pragma unroll
     for (int o = C; o < 32; o <<= 1) sum += __shfl_xor_sync(FULL, sum, o);
     __syncwarp();
