@@ -71,7 +71,7 @@ class ClockSampler:
         0x100: "display_clock_setting", 0x10: "sync_boost",
     }
 
-    def __init__(self, torch_device_index: int, period_s: float = 0.02):
+    def __init__(self, torch_device_index: int, period_s: float = 0.001):
         self.period = period_s
         self.samples: list[int] = []
         self.reason_bits = 0
@@ -309,16 +309,22 @@ def run_cuda(args) -> None:
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     achieved_tf = executed * flop_per_term / t_tr / 1e12
 
-    # measured DFMA ceiling of this device, same process (dependent chains, 8 per thread)
+    # measured FP64 ceilings of this device, same process (libgcamb_probe.so, not part of the method):
+    # dependent DFMA chains (8 per thread) and mma.sync.m8n8k4.f64 chains (8 per warp, 256 FMA each)
     probe_out = torch.empty(n_sm * 8 * 256, dtype=torch.float64, device=dev)
     iters = 1 << 14
-    los.gcamb_los_dfma_probe(n_sm * 8, 256, iters, probe_out)
-    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    p0.record()
-    los.gcamb_los_dfma_probe(n_sm * 8, 256, iters, probe_out)
-    p1.record()
-    torch.cuda.synchronize()
-    probe_tf = n_sm * 8 * 256 * 8 * iters * 2 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    def probe_tflops(fn, fma_per_thread_iter):
+        fn(n_sm * 8, 256, iters, probe_out)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record()
+        fn(n_sm * 8, 256, iters, probe_out)
+        p1.record()
+        torch.cuda.synchronize()
+        return n_sm * 8 * 256 * fma_per_thread_iter * iters * 2 / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    probe_tf = probe_tflops(los.gcamb_probe_dfma, 8)
+    probe_dmma_tf = probe_tflops(los.gcamb_probe_dmma, 8 * 256 / 32)
 
     if rank != 0:
         if dist is not None:
@@ -347,7 +353,8 @@ def run_cuda(args) -> None:
             "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
             "traffic_unit": "bytes per transfer call (ncu dram read+write, profiles/r1_transfer_kernel_*.txt)",
             "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
-                           f"dfma probe measured {probe_tf:.2f} TFLOP/s in this process",
+                           f"dfma probe measured {probe_tf:.2f} TFLOP/s, dmma (m8n8k4.f64) probe "
+                           f"{probe_dmma_tf:.2f} TFLOP/s in this process",
             "algorithmic": f"{flop_per_term} flop per executed term x {executed} executed terms per launch",
             "frac_of_measured_dfma": achieved_tf / probe_tf,
         },

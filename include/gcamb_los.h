@@ -55,18 +55,21 @@ enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4 };
  * of the downward j_l recurrence: the first l-tile that is not negligible (R16: j_l(x) := 0 for
  * l above ~ x + 18.2 x^(1/3) + 8, where |j_l| < 1e-36) and the normalised pair
  * (j_{l+1}(x), j_l(x)) at the top of that tile, generated ON THE DEVICE by Miller's backward
- * recurrence normalised against closed-form j_0 and j_1 (BJ (b), R15).  That is 20 bytes per
- * (k, tau) point -- O(N_k N_tau), not an O(N_l N_k N_tau) j_l table.  Also sorts k by cost so
- * that the heaviest blocks are issued first.
+ * recurrence normalised against closed-form j_0 and j_1 (BJ (b), R15).  With the tile index and
+ * 1/x that is 28 bytes per (k, tau) point -- O(N_k N_tau), not an O(N_l N_k N_tau) j_l table.
+ * Also sorts k by cost so that the heaviest blocks are issued first.
  *
  *   l_list  HOST [n_l]   strictly increasing, 2 <= l <= 65535 (any subset; the recurrence walks
  *                        every l, only listed l are stored; stretches of 8 l without a listed l
  *                        cost the recurrence only, about half the time of a listed stretch, R21)
- *   k       HOST [n_k]   strictly increasing, > 0, finite; n_k >= 2
+ *   k       HOST [n_k]   strictly increasing, > 0, finite; n_k >= 2 (and n_k * n_batch < 2^31 in
+ *                        the batched calls: one thread block per k row and cosmology)
  *   tau     HOST [n_tau] strictly increasing, < tau0, finite; n_tau >= 2
  *   src_mask             GCAMB_SRC_T|GCAMB_SRC_E or GCAMB_SRC_T|GCAMB_SRC_E|GCAMB_SRC_PHI
  *   cuda_stream          stream the precompute kernels run on; the call synchronises it.
  * On success *out owns device memory on the CURRENT device; free with gcamb_los_plan_destroy.
+ * Every later call on the plan must be made with that device current (GCAMB_EINVAL otherwise;
+ * gcamb_los_plan_destroy switches to it and back by itself).
  */
 gcamb_status gcamb_los_plan_create(gcamb_los_plan **out,
                                    const int32_t *l_list, int32_t n_l,
@@ -91,8 +94,9 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
  * Kernels of this library that one gcamb_los_transfer[_batched] call and one gcamb_los_cls[_batched]
  * call launch on this plan (any batch size).  The transfer is one launch, or two overlapping ones when
  * only some rows (x_max = k (tau0 - tau_0) > 2^53 * 7.5e-13 = 6755) take the compensated recurrence
- * coefficient; a cudaMemsetAsync of Delta precedes them when the
- * tau grid is split over several CTAs per k.  Either pointer may be NULL.
+ * coefficient.  Nothing else is enqueued: no memset, no atomics;
+ * tau grids longer than one thread block's slots are taken in passes by the same block, so results
+ * are bit-reproducible for any n_tau.  Either pointer may be NULL.
  */
 gcamb_status gcamb_los_plan_launches(const gcamb_los_plan *plan, int32_t *transfer_kernels,
                                      int32_t *cls_kernels);
@@ -147,14 +151,6 @@ gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch,
                                     const double *h_S_T, const double *h_S_E, const double *h_S_phi,
                                     const double *h_P_R, double *h_Cl, double *h_Delta,
                                     void *cuda_stream);
-
-/*
- * Roofline denominator helper: enqueues a pure dependent-chain DFMA kernel (8 independent chains
- * per thread, `iters` FMAs per chain) on `cuda_stream`.  The caller times it with CUDA events;
- * it performs exactly  blocks * threads * 8 * iters  DFMAs.  d_out DEVICE [blocks*threads].
- */
-gcamb_status gcamb_los_dfma_probe(int32_t blocks, int32_t threads, int64_t iters, double *d_out,
-                                  void *cuda_stream);
 
 /* Thread-local message of the last non-OK status on this thread ("" if none). */
 const char *gcamb_los_last_error(void);

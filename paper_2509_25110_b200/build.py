@@ -1,4 +1,5 @@
-"""Builds libgcamb_los.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+"""Builds libgcamb_los.so (the product) and libgcamb_probe.so (bench.py's roofline probes, not part
+of the method) in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2509_25110_b200.build [--force] [--verbose]
 """
@@ -15,6 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgcamb_los.so")
+PROBE_LIB = os.path.join(HERE, "libgcamb_probe.so")
 # (source, extra flags, object tag): transfer.cu is compiled once per (sparse, n_src) entry, in parallel
 UNITS = [("api.cu", [], "api"), ("plan.cu", [], "plan"), ("cls.cu", [], "cls")] + [
     ("transfer.cu", [f"-DGCAMB_TU_SPARSE={sp}", f"-DGCAMB_TU_NSRC={ns}"], f"transfer_s{sp}n{ns}")
@@ -27,10 +29,11 @@ NVCC_FLAGS = [
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not (os.path.exists(LIB) and os.path.exists(PROBE_LIB)):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "gcamb_los.h"), __file__]
+    t = min(os.path.getmtime(LIB), os.path.getmtime(PROBE_LIB))
+    inc = os.path.join(ROOT, "include")
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(inc, f) for f in os.listdir(inc)] + [__file__]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -48,13 +51,17 @@ def build_extension(force: bool = False, verbose: bool = False) -> str:
                    "-c", os.path.join(CSRC, src), "-o", obj]
             subprocess.run(cmd, check=True)
             return obj
-        with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 1)) as pool:
+        with ThreadPoolExecutor(max_workers=min(len(UNITS) + 1, os.cpu_count() or 1)) as pool:
+            probe = pool.submit(compile_unit, ("probe.cu", [], "probe"))
             objs = list(pool.map(compile_unit, UNITS))
-        tmp = f"{LIB}.{os.getpid()}.tmp"
-        subprocess.run([nvcc, "-shared", "-cudart", "shared", "-gencode", "arch=compute_100a,code=sm_100a",
-                        *objs, "-o", tmp], check=True)
+            probe_obj = probe.result()
+        link = [nvcc, "-shared", "-cudart", "shared", "-gencode", "arch=compute_100a,code=sm_100a"]
+        tmp, tmp_probe = f"{LIB}.{os.getpid()}.tmp", f"{PROBE_LIB}.{os.getpid()}.tmp"
+        subprocess.run([*link, *objs, "-o", tmp], check=True)
+        subprocess.run([*link, probe_obj, "-o", tmp_probe], check=True)
     finally:
         shutil.rmtree(objdir, ignore_errors=True)
+    os.replace(tmp_probe, PROBE_LIB)
     os.replace(tmp, LIB)
     return LIB
 

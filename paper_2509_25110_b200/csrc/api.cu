@@ -62,10 +62,23 @@ static void free_plan(gcamb_los_plan *p)
     delete p;
 }
 
+// a plan's tables live on the device that was current at its creation; so must the caller's buffers
+static gcamb_status check_device(const gcamb_los_plan *p)
+{
+    int dev = -1;
+    GCAMB_CUDA(cudaGetDevice(&dev));
+    if (dev != p->device) {
+        set_error("plan belongs to device %d but device %d is current", p->device, dev);
+        return GCAMB_EINVAL;
+    }
+    return GCAMB_OK;
+}
+
 static gcamb_status check_call(const gcamb_los_plan *p, int n_batch, const double *S_T,
                                const double *S_E, const double *S_phi, const void *out)
 {
     if (!p || !S_T || !S_E || !out) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(p)) return st;
     if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
     if ((long long)p->n_k * n_batch > 0x7fffffffLL) {   // one CTA per (k, cosmology) along grid.x
         set_error("n_k * n_batch must be below 2^31");
@@ -93,7 +106,6 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (out) *out = nullptr;
     if (!out || !l_list || !k || !tau) { set_error("null argument"); return GCAMB_EINVAL; }
     if (n_l < 1 || n_k < 2 || n_tau < 2) { set_error("need n_l >= 1, n_k >= 2, n_tau >= 2"); return GCAMB_EINVAL; }
-    if (n_k > 65535) { set_error("n_k must be <= 65535"); return GCAMB_EINVAL; }
     if (src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
         set_error("src_mask must be T|E or T|E|PHI");
         return GCAMB_EINVAL;
@@ -121,9 +133,12 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     p->n_spec = p->n_src + 1;
     p->l_min = l_list[0]; p->l_max = l_list[n_l - 1];
     p->tau0 = tau0;
-    p->shape = choose_shape(n_tau, p->n_src);
-    p->n_tiles = (p->l_max - p->l_min) / p->shape.V + 1;
     cudaStream_t stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
+    if (e != cudaSuccess) { gcamb_status st = cuda_fail(e, "device query"); free_plan(p); return st; }
+    p->shape = choose_shape(n_tau, p->n_src, n_k, p->n_sm);
+    p->n_tiles = (p->l_max - p->l_min) / p->shape.V + 1;
 
     // IntegrationVars_init: the O(N) tables, on the host in fp64
     std::vector<double> vk(k, k + n_k), vtau(tau, tau + n_tau), chi(n_tau), lnk(n_k), pref(n_l);
@@ -137,8 +152,7 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
         pref[i] = std::sqrt((l + 2.0) * (l + 1.0) * l * (l - 1.0));   // (l+2)!/(l-2)!  (R3)
     }
 
-    cudaError_t e = cudaGetDevice(&p->device);
-    if (e == cudaSuccess) e = upload(&p->d_l_index, l_index, stream);
+    e = upload(&p->d_l_index, l_index, stream);
     if (e == cudaSuccess) e = upload(&p->d_l_list, std::vector<int32_t>(l_list, l_list + n_l), stream);
     {   // sparse l lists: which tiles hold a listed l (NULL table = all of them)
         std::vector<uint32_t> mask((p->n_tiles + 31) / 32, 0u);
@@ -173,8 +187,14 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
 gcamb_status gcamb_los_plan_destroy(gcamb_los_plan *plan)
 {
     if (!plan) return GCAMB_OK;
-    cudaError_t e = cudaDeviceSynchronize();
+    // synchronise and free on the owning device, whatever device is current; restore the caller's
+    int cur = -1;
+    const int owner = plan->device;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e == cudaSuccess && cur != owner) e = cudaSetDevice(owner);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
     free_plan(plan);
+    if (cur >= 0 && cur != owner) cudaSetDevice(cur);
     if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceSynchronize");
     return GCAMB_OK;
 }
@@ -220,6 +240,7 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch, 
 {
     if (!plan || !d_Delta || !d_P_R || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
     if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(plan)) return st;
     return launch_cls(plan, n_batch, d_Delta, d_P_R, d_Cl, (cudaStream_t)cuda_stream);
 }
 
@@ -229,15 +250,14 @@ gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, co
     return gcamb_los_cls_batched(plan, 1, d_Delta, d_P_R, d_Cl, cuda_stream);
 }
 
-gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const double *h_S_T,
-                                    const double *h_S_E, const double *h_S_phi, const double *h_P_R,
-                                    double *h_Cl, double *h_Delta, void *cuda_stream)
+}  // extern "C"
+
+// everything gcamb_los_spectra_host enqueues; on an error the caller joins the streams before returning
+static gcamb_status spectra_host_enqueue(gcamb_los_plan *p, int32_t n_batch, const double *h_S_T,
+                                         const double *h_S_E, const double *h_S_phi, const double *h_P_R,
+                                         double *h_Cl, double *h_Delta, cudaStream_t s)
 {
-    gcamb_status st = check_call(plan, n_batch, h_S_T, h_S_E, h_S_phi, h_Cl);
-    if (st != GCAMB_OK) return st;
-    if (!h_P_R) { set_error("null P_R"); return GCAMB_EINVAL; }
-    gcamb_los_plan *p = plan;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
+    gcamb_status st;
     const size_t nS = (size_t)p->n_k * p->n_tau, nD = (size_t)p->n_src * p->n_l * p->n_k;
     const size_t nC = (size_t)p->n_spec * p->n_l;
     if (n_batch > p->host_batch_cap) {
@@ -271,8 +291,6 @@ gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const
         }
         p->h_streams_ready = 1;
     }
-    st = launch_transfer_prepare(p, n_batch, p->d_hDelta, s);
-    if (st != GCAMB_OK) return st;
     if (!pipelined) {
         for (int q = 0; q < p->n_src; ++q)
             GCAMB_CUDA(cudaMemcpyAsync(p->d_hS[q], hS[q], sizeof(double) * nS * n_batch, cudaMemcpyHostToDevice, s));
@@ -305,35 +323,35 @@ gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const
     GCAMB_CUDA(cudaMemcpyAsync(h_Cl, p->d_hCl, sizeof(double) * nC * n_batch, cudaMemcpyDeviceToHost, s));
     if (h_Delta)
         GCAMB_CUDA(cudaMemcpyAsync(h_Delta, p->d_hDelta, sizeof(double) * nD * n_batch, cudaMemcpyDeviceToHost, s));
-    GCAMB_CUDA(cudaStreamSynchronize(s));
+    return GCAMB_OK;
+}
+
+extern "C" {
+
+gcamb_status gcamb_los_spectra_host(gcamb_los_plan *plan, int32_t n_batch, const double *h_S_T,
+                                    const double *h_S_E, const double *h_S_phi, const double *h_P_R,
+                                    double *h_Cl, double *h_Delta, void *cuda_stream)
+{
+    gcamb_status st = check_call(plan, n_batch, h_S_T, h_S_E, h_S_phi, h_Cl);
+    if (st != GCAMB_OK) return st;
+    if (!h_P_R) { set_error("null P_R"); return GCAMB_EINVAL; }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    st = spectra_host_enqueue(plan, n_batch, h_S_T, h_S_E, h_S_phi, h_P_R, h_Cl, h_Delta, s);
+    // Join every stream the call may have used, also on the error path: asynchronous copies from and to
+    // the caller's buffers must not be in flight when the call returns.
+    cudaError_t e = cudaStreamSynchronize(s);
+    if (plan->h_streams_ready) {
+        cudaError_t e2 = cudaStreamSynchronize(plan->h_copy);
+        if (e == cudaSuccess) e = e2;
+        for (int c = 0; c < 4; ++c) {
+            e2 = cudaStreamSynchronize(plan->h_comp[c]);
+            if (e == cudaSuccess) e = e2;
+        }
+    }
+    if (st != GCAMB_OK) return st;
+    if (e != cudaSuccess) return cuda_fail(e, "gcamb_los_spectra_host: stream synchronisation");
     return GCAMB_OK;
 }
 
 }  // extern "C"
 
-// ------------------------------------------------------------------ DFMA roofline probe
-namespace gcamb {
-__global__ void dfma_probe_kernel(long long iters, double *out)
-{
-    double a[8], m = 1.0 - 1e-9 * (threadIdx.x & 7), c = 1e-12;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) a[q] = 1.0 + q;
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int q = 0; q < 8; ++q) a[q] = fma(a[q], m, c);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) s += a[q];
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-}  // namespace gcamb
-
-extern "C" gcamb_status gcamb_los_dfma_probe(int32_t blocks, int32_t threads, int64_t iters, double *d_out,
-                                             void *cuda_stream)
-{
-    if (blocks < 1 || threads < 1 || threads > 1024 || iters < 1 || !d_out) { set_error("bad probe arguments"); return GCAMB_EINVAL; }
-    gcamb::dfma_probe_kernel<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>((long long)iters, d_out);
-    GCAMB_CUDA(cudaGetLastError());
-    return GCAMB_OK;
-}

@@ -1,64 +1,113 @@
 // cls.cu -- step a4: C_l^{XY} = 4 pi sum_j dlnk_j P_R(k_j) Delta^X_l(k_j) Delta^Y_l(k_j)
 // (Eq. 1; discrete form BJ, R6, R12).  HBM-bound: Delta is read exactly once,
-// coalesced along k; one CTA per (l, cosmology); fixed-order (deterministic) block reduction.
+// coalesced along k with 16-byte loads.  One CTA takes R consecutive l of one cosmology, so that
+// the weights w_j = dlnk_j P_R(k_j) are formed once per R rows (at one row per CTA the weight reads
+// doubled the L2 -> SM traffic) and every thread has 2 + R n_src independent loads in flight per
+// step.  Fixed-order (deterministic) reduction: thread-private sums over k, shuffle tree, then the
+// warps in index order.
 #include "los_internal.cuh"
 
 namespace gcamb {
 
 constexpr int CLS_THREADS = 256;
 
-template <int NSRC>
+template <int VEC> struct Pack;
+template <> struct Pack<1> { double v[1]; };
+template <> struct alignas(16) Pack<2> { double v[2]; };
+
+template <int NSRC, int R, int VEC>
 __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restrict__ Delta,
                                                           const double *__restrict__ P_R,
                                                           const double *__restrict__ dlnk,
                                                           double *__restrict__ Cl, int n_l, int n_k)
 {
     constexpr int NSPEC = NSRC + 1;
-    const int li = blockIdx.x, b = blockIdx.y;
-    const double *dT = Delta + (((size_t)b * NSRC + 0) * n_l + li) * n_k;
-    const double *dE = Delta + (((size_t)b * NSRC + 1) * n_l + li) * n_k;
-    const double *dP = NSRC == 3 ? Delta + (((size_t)b * NSRC + 2) * n_l + li) * n_k : nullptr;
-    const double *pr = P_R + (size_t)b * n_k;
-    double s[NSPEC];
+    using pack = Pack<VEC>;
+    const int l0 = blockIdx.x * R, b = blockIdx.y;
+    const pack *row[R][NSRC];
 #pragma unroll
-    for (int q = 0; q < NSPEC; ++q) s[q] = 0.0;
-    for (int j = threadIdx.x; j < n_k; j += CLS_THREADS) {
-        const double wp = dlnk[j] * pr[j];
-        const double t = dT[j], e = dE[j];
-        s[0] = fma(wp * t, t, s[0]);
-        s[1] = fma(wp * e, e, s[1]);
-        s[2] = fma(wp * t, e, s[2]);
-        if (NSRC == 3) {
-            const double ph = dP[j];
-            s[NSPEC - 1] = fma(wp * ph, ph, s[NSPEC - 1]);
+    for (int r = 0; r < R; ++r) {
+        const int li = min(l0 + r, n_l - 1);   // rows past the end re-read the last one and are dropped below
+#pragma unroll
+        for (int q = 0; q < NSRC; ++q)
+            row[r][q] = reinterpret_cast<const pack *>(Delta + (((size_t)b * NSRC + q) * n_l + li) * n_k);
+    }
+    const pack *pr = reinterpret_cast<const pack *>(P_R + (size_t)b * n_k);
+    const pack *dl = reinterpret_cast<const pack *>(dlnk);
+    double s[R][NSPEC];
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int q = 0; q < NSPEC; ++q) s[r][q] = 0.0;
+    const int n_pack = n_k / VEC;
+#pragma unroll 2
+    for (int j = threadIdx.x; j < n_pack; j += CLS_THREADS) {
+        const pack a = dl[j], c = pr[j];
+        pack d[R][NSRC];
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int q = 0; q < NSRC; ++q) d[r][q] = row[r][q][j];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            const double wp = a.v[v] * c.v[v];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double t = d[r][0].v[v], e = d[r][1].v[v];
+                s[r][0] = fma(wp * t, t, s[r][0]);
+                s[r][1] = fma(wp * e, e, s[r][1]);
+                s[r][2] = fma(wp * t, e, s[r][2]);
+                if (NSRC == 3) {
+                    const double ph = d[r][NSRC - 1].v[v];
+                    s[r][NSPEC - 1] = fma(wp * ph, ph, s[r][NSPEC - 1]);
+                }
+            }
         }
     }
-    __shared__ double sm[NSPEC][CLS_THREADS / 32];
+    __shared__ double sm[R * NSPEC][CLS_THREADS / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-    for (int q = 0; q < NSPEC; ++q) {
-        double v = s[q];
+    for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) sm[q][warp] = v;
-    }
+        for (int q = 0; q < NSPEC; ++q) {
+            double v = s[r][q];
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) sm[r * NSPEC + q][warp] = v;
+        }
     __syncthreads();
-    if (threadIdx.x < NSPEC) {
-        double v = 0.0;
+    if (threadIdx.x < R * NSPEC) {
+        const int r = threadIdx.x / NSPEC, q = threadIdx.x - r * NSPEC;
+        if (l0 + r < n_l) {
+            double v = 0.0;
 #pragma unroll
-        for (int wv = 0; wv < CLS_THREADS / 32; ++wv) v += sm[threadIdx.x][wv];
-        Cl[((size_t)b * NSPEC + threadIdx.x) * n_l + li] = 4.0 * 3.14159265358979323846 * v;
+            for (int wv = 0; wv < CLS_THREADS / 32; ++wv) v += sm[threadIdx.x][wv];
+            Cl[((size_t)b * NSPEC + q) * n_l + l0 + r] = 4.0 * 3.14159265358979323846 * v;
+        }
     }
+}
+
+template <int NSRC, int R>
+static void launch_rows(bool vec, dim3 grid, cudaStream_t stream, const double *Delta, const double *P_R,
+                        const double *dlnk, double *Cl, int n_l, int n_k)
+{
+    if (vec) cls_kernel<NSRC, R, 2><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
+    else cls_kernel<NSRC, R, 1><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
 }
 
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,
                         const double *P_R, double *Cl, cudaStream_t stream)
 {
-    dim3 grid((unsigned)p->n_l, (unsigned)n_batch);
-    if (p->n_src == 2)
-        cls_kernel<2><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k);
-    else
-        cls_kernel<3><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k);
+    // 16-byte loads need even rows and aligned bases (every row then starts on a 16-byte boundary)
+    const bool vec = p->n_k % 2 == 0 && ((uintptr_t)Delta | (uintptr_t)P_R) % 16 == 0;
+    // rows per CTA: 4 while that still leaves two CTAs per SM, else 2, else 1
+    int R = 4;
+    while (R > 1 && (long long)((p->n_l + R - 1) / R) * n_batch < 2LL * p->n_sm) R >>= 1;
+    dim3 grid((unsigned)((p->n_l + R - 1) / R), (unsigned)n_batch);
+#define GCAMB_CLS(NS, RR) launch_rows<NS, RR>(vec, grid, stream, Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k)
+    if (p->n_src == 2) { if (R == 4) GCAMB_CLS(2, 4); else if (R == 2) GCAMB_CLS(2, 2); else GCAMB_CLS(2, 1); }
+    else               { if (R == 4) GCAMB_CLS(3, 4); else if (R == 2) GCAMB_CLS(3, 2); else GCAMB_CLS(3, 1); }
+#undef GCAMB_CLS
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
 }

@@ -14,7 +14,8 @@ struct TransferShape {
     int V;        // l-tile: accumulators per source per thread, = granularity of start tiles
     int T;        // (k, tau) points ("slots") carried per thread
     int threads;  // CTA size (multiple of 32)
-    int n_split;  // CTAs sharing one k along tau (1 = plain stores, >1 = fp64 RED into zeroed Delta)
+    int n_pass;   // passes of one CTA over the tau range (n_tau > threads * T: pass p adds to passes < p)
+    int pass_len; // tau points per pass (the last pass may be shorter)
 };
 
 }  // namespace gcamb
@@ -27,7 +28,8 @@ struct gcamb_los_plan {
     int64_t executed_terms;  // sum over (k,tau) of #l in [l_min, min(L(x), l_max)]
     int32_t n_comp;          // leading positions of korder that run the compensated coefficient (transfer.cu)
     int64_t walked_terms;    // same with the tile-aligned start the kernel really walks
-    int device;
+    int device;              // the device that owns the tables; every call checks it is the current one
+    int n_sm;                // its SM count
 
     // device tables
     int32_t *d_l_index;  // [l_max+1] position in l_list, or -1
@@ -42,7 +44,7 @@ struct gcamb_los_plan {
     int32_t *d_korder;   // [n_k] k indices, heaviest first
     int32_t *d_l_list;   // [n_l] the l list
     uint32_t *d_tile_mask;   // [ceil(n_tiles/32)] bit t%32 of word t/32: tile t holds a listed l; NULL when every tile does
-    int32_t *d_kz;       // [n_tiles] #k whose walk starts below tile t: Delta rows of tile t are 0 for k < kz[t]; NULL if not monotone
+    int32_t *d_kz;       // [n_tiles] #k whose walk starts below tile t: Delta rows of tile t are 0 for k < kz[t]
 
     int32_t order_reversed;  // korder[r] == n_k - 1 - r: a range of positions is a contiguous range of k
 
@@ -71,17 +73,16 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream);
 // transfer.cu
 // x above which the systematic phase error x 2^-53 of the rounded reciprocal exceeds 7.5e-13 rad
 //
-#ifndef GCAMB_COMP_X_MIN
-#define GCAMB_COMP_X_MIN 6755.399441055744   // 2^53 * 7.5e-13
-#endif
-constexpr double COMP_X_MIN = GCAMB_COMP_X_MIN;
-TransferShape choose_shape(int n_tau, int n_src);
+constexpr double COMP_X_MIN = 6755.399441055744;   // 2^53 * 7.5e-13
+int transfer_tile_v();
+// n_rows = the k rows of ONE cosmology (a batched call must take the shape of the single call)
+TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm);
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,
                              cudaStream_t stream);
-// the same in pieces, for the pipelined host entry point: `prepare` once, then any partition of the
-// cost-order positions [0, n_k) into ranges, exactly one of them (any) with zero_fill
-gcamb_status launch_transfer_prepare(const gcamb_los_plan *p, int n_batch, double *Delta, cudaStream_t stream);
+// the same in pieces, for the pipelined host entry point: any partition of the cost-order positions
+// [0, n_k) into ranges, exactly one of them (any) with zero_fill (that range zeroes the skipped
+// region of ALL rows)
 gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
                                    const double *S_E, const double *S_phi, double *Delta,
                                    int pos0, int pos1, bool zero_fill, cudaStream_t stream);

@@ -43,8 +43,8 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
                                                            int32_t *__restrict__ tile,
                                                            double *__restrict__ inv_x)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;   // k along grid.x: n_k is bounded by 2^31 - 1 only
+    const int j = blockIdx.x;
     if (i >= n_tau) return;
     const double x = __dmul_rn(k[j], chi[i]);
     const int L = l_cut(x);
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ 
 gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
 {
     const int V = p->shape.V;
-    dim3 grid((p->n_tau + 127) / 128, p->n_k);
+    dim3 grid(p->n_k, (p->n_tau + 127) / 128);
     start_values_kernel<<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V,
                                                   p->d_start, p->d_tile, p->d_inv);
     GCAMB_CUDA(cudaGetLastError());
@@ -168,21 +168,24 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     }
     // zero region of Delta (R16): x grows with k, so the first tile of a k (that of tau_0, its
     // largest x) never rises with k, and the rows of tile t are exactly zero for the first kz[t]
-    // k.  If the first tiles were ever not monotone the kernel falls back to per-CTA zero stores.
+    // k: the transfer kernel zeroes those row prefixes with coalesced stores.  The first tiles are
+    // monotone for any valid (strictly increasing) k grid because L(x) is monotone in x; anything
+    // else is an internal error and is reported, not worked around.
     const long long *first = cost.data() + 2 * (size_t)p->n_k;
-    bool monotone = true;
-    for (int j = 1; j < p->n_k; ++j) monotone = monotone && first[j] <= first[j - 1];
-    p->d_kz = nullptr;
-    if (monotone) {
-        std::vector<int32_t> kz(p->n_tiles);
-        int j = p->n_k;   // kz[t] = #{k : first[k] > t}, non-increasing in t
-        for (int t = 0; t < p->n_tiles; ++t) {
-            while (j > 0 && first[j - 1] <= t) --j;
-            kz[t] = j;
+    for (int j = 1; j < p->n_k; ++j) {
+        if (first[j] > first[j - 1]) {
+            set_error("internal: first l-tile not monotone in k at k index %d", j);
+            return GCAMB_EGRID;
         }
-        GCAMB_CUDA(cudaMalloc(&p->d_kz, sizeof(int32_t) * p->n_tiles));
-        GCAMB_CUDA(cudaMemcpyAsync(p->d_kz, kz.data(), sizeof(int32_t) * p->n_tiles, cudaMemcpyHostToDevice, stream));
     }
+    std::vector<int32_t> kz(p->n_tiles);
+    int j = p->n_k;   // kz[t] = #{k : first[k] > t}, non-increasing in t
+    for (int t = 0; t < p->n_tiles; ++t) {
+        while (j > 0 && first[j - 1] <= t) --j;
+        kz[t] = j;
+    }
+    GCAMB_CUDA(cudaMalloc(&p->d_kz, sizeof(int32_t) * p->n_tiles));
+    GCAMB_CUDA(cudaMemcpyAsync(p->d_kz, kz.data(), sizeof(int32_t) * p->n_tiles, cudaMemcpyHostToDevice, stream));
     GCAMB_CUDA(cudaStreamSynchronize(stream));
     return GCAMB_OK;
 }

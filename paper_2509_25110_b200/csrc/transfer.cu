@@ -1,6 +1,6 @@
 // transfer.cu -- steps a1-a3 of the hot path: sources -> Delta^X_l(k)  (Eq. 2-3).
 //
-// Mapping: one CTA per k (per tau-split), lanes <-> consecutive tau.
+// Mapping: one CTA per k, lanes <-> consecutive tau.
 // Every thread carries T (k,tau) points ("slots") whose recurrence state lives in registers for
 // the whole walk: f_{l+1}, f_l, 1/x and the pre-weighted sources s_X = w S_X (s_E also / x^2).
 // The CTA walks l DOWNWARD in tiles of V; per point and l it issues
@@ -17,11 +17,16 @@
 //
 // Reduction: after a tile the V x n_src per-thread sums are reduced across the warp through a
 // shared-memory transpose (1 DADD per l and source, no shuffles or selects) into a ring;
-// every G tiles the CTA synchronises once, sums the warps in fixed order, applies the Delta^E
-// prefactor and stores.  The summation order is fixed by the launch shape alone, so results are
-// bit-reproducible and the batched call equals a loop of single calls.
+// every G tiles the warps' entries are summed in fixed order, the Delta^E prefactor is applied and
+// the result stored.
+//
+// tau ranges longer than one CTA's slots (n_tau > threads * T) are taken in PASSES by the same CTA:
+// pass 0 stores its sums, pass p > 0 adds its own to what the CTA stored before (plain loads and
+// stores of its own k column, ordered by a CTA barrier).  No atomics, no cleared output buffer: the
+// order of every sum is fixed by (n_tau, n_src) alone, so results are bit-reproducible run to run,
+// a k row does not depend on the other rows, and the batched call equals a loop of single calls.
 #include <algorithm>
-
+#include <atomic>
 #include <cassert>
 
 #include "los_internal.cuh"
@@ -44,13 +49,14 @@ struct TransferParams {
     const double2 *start;
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     const uint32_t *tile_mask;   // [ceil(n_tiles/32)] bit = the tile holds an l of the list (sparse lists only)
-    int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_split, split_len;
+    int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_pass, pass_len;
     int order_reversed;   // korder[r] == n_k - 1 - r
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
     int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
     int zero_fill;  // this launch also zeroes the skipped region of Delta (all rows of it)
 };
 
+constexpr int T_MAX = 12;      // points per thread: the NA dispatch of the kernel is written out up to 12
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int NEVER = 0x7fffffff;
 
@@ -112,6 +118,10 @@ constexpr int LAG = 1;   // a group is flushed this many groups after it was wri
 __device__ __forceinline__ void mbar_init(uint32_t bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_inval(uint32_t bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
@@ -190,7 +200,7 @@ __device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T]
 template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
-    static_assert(T >= 1 && T <= 12, "the NA dispatch below is written out for T <= 12");
+    static_assert(T >= 1 && T <= T_MAX, "the NA dispatch below is written out for T <= 12");
     constexpr int P = NSRC * V;          // partial sums per thread and tile
     constexpr int NOUT = (G * P + MAXTHREADS - 1) / MAXTHREADS;   // flush outputs per thread (full CTA)
     // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] |
@@ -213,18 +223,28 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const int bid = blockIdx.x;
     // The compensated rows run as their own small launch; the launch after it carries the
     // programmatic-stream-serialization attribute and may start as soon as every CTA of this one has
-    // passed this point (the two launches write disjoint rows of Delta and never wait on each other).
+    // passed this point (the two launches write disjoint rows of Delta and never wait on each other;
+    // the dependent launch waits for this one at its very end, see griddepcontrol.wait below).
     asm volatile("griddepcontrol.launch_dependents;");
     const int krel = bid / p.n_batch, b = bid - krel * p.n_batch;
     const int krank = p.k_first + krel;   // position in the cost order
     constexpr bool comp = COMP;           // this launch takes the compensated coefficient
     // the cost order is the k grid reversed whenever cost grows with k: no table look-up then
     const int kidx = p.order_reversed ? p.n_k - 1 - krank : __reduce_min_sync(0xffffffffu, p.korder[krank]);   // uniform register, like the bookkeeping below
-    const int split = blockIdx.y;
-    const int i_begin = split * p.split_len;
-    const int i_end = min(p.n_tau, i_begin + p.split_len);
     const double kval = p.k[kidx];
     const size_t row = (size_t)kidx * p.n_tau;
+    const size_t delta_b = (size_t)b * NSRC * p.n_l;
+#define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
+
+  for (int pass = 0; pass < p.n_pass; ++pass) {
+    if (pass) {   // the ring and its barriers start afresh; the stores of the previous pass are visible to the whole CTA
+        __syncthreads();
+        if (tid == 0)
+            for (int d = 0; d < 2 * RD; ++d) { mbar_inval(bar_full + 8 * d); mbar_init(bar_full + 8 * d, W); }
+        __syncthreads();
+    }
+    const int i_begin = pass * p.pass_len;
+    const int i_end = min(p.n_tau, i_begin + p.pass_len);
 
     // ---- a1: source staging.  Slot j of the CTA covers tau indices i_begin + j*blockDim ...
     // + blockDim - 1 in W chunks of 32 consecutive tau ("ranks"; rank 0 has the largest x and the
@@ -236,7 +256,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // zero-prefix lengths of the (at most two, normally) Delta rows this CTA zero-fills: looked up here
     // so that the look-ups travel with the prologue loads instead of adding their own round trips
     const int zf_rows = NSRC * p.n_l, zf_step = gridDim.x / p.n_batch;
-    const bool zf = p.n_split == 1 && p.zero_fill && p.kz != nullptr;
+    const bool zf = pass == 0 && p.zero_fill;
     int zf_nz[2] = {0, 0};
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
@@ -287,33 +307,21 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     __syncwarp();
 
     const int t_begin = __reduce_min_sync(FULL, t_begin_load);
-    const size_t delta_b = (size_t)b * NSRC * p.n_l;
-#define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
 
     // l above the first tile of a k: Delta is exactly zero there (R16).  Those elements form, for
-    // every l, a prefix k < kz[tile of l] of the Delta row, so the CTAs share the rows among
-    // themselves and zero them with coalesced stores (a CTA's own zero elements lie along l, 8 bytes
-    // every n_k doubles).  With RED output the launcher zeroed the whole buffer instead.
-    if (p.n_split == 1 && p.zero_fill) {
-        if (p.kz) {
-            int u = 0;
-            for (int r = krel; r < zf_rows; r += zf_step, ++u) {
-                const int li = r % p.n_l;
-                const int nz = u < 2 ? zf_nz[u < 1 ? 0 : 1]
-                                     : p.kz[(p.l_max - (p.l_contig ? p.l_min + li : p.l_list[li])) / V];
-                double *dst = p.Delta + (delta_b + r) * p.n_k;
-                GCAMB_ASSERT(nz >= 0 && nz <= p.n_k && r < zf_rows && li < p.n_l);
-                for (int j = tid; j < nz; j += blockDim.x) dst[j] = 0.0;
-            }
-        } else {
-            const int l_top = max(p.l_max - t_begin * V, p.l_min - 1);  // highest l walked
-            for (int l = p.l_max - tid; l > l_top; l -= blockDim.x) {
-                const int li = p.l_contig ? l - p.l_min : p.l_index[l];
-                if (li >= 0) {
-#pragma unroll
-                    for (int q = 0; q < NSRC; ++q) p.Delta[DIDX(q, li)] = 0.0;
-                }
-            }
+    // every l, a prefix k < kz[tile of l] of the Delta row (x grows with k, so the first tile of a k
+    // never rises with k: checked at plan creation), so the CTAs share the rows among themselves and
+    // zero them with coalesced stores (a CTA's own zero elements lie along l, 8 bytes every n_k
+    // doubles).  Later passes (smaller x) start at or below the first tile of pass 0.
+    if (zf) {
+        int u = 0;
+        for (int r = krel; r < zf_rows; r += zf_step, ++u) {
+            const int li = r % p.n_l;
+            const int nz = u < 2 ? zf_nz[u < 1 ? 0 : 1]
+                                 : p.kz[(p.l_max - (p.l_contig ? p.l_min + li : p.l_list[li])) / V];
+            double *dst = p.Delta + (delta_b + r) * p.n_k;
+            GCAMB_ASSERT(nz >= 0 && nz <= p.n_k && r < zf_rows && li < p.n_l);
+            for (int j = tid; j < nz; j += blockDim.x) dst[j] = 0.0;
         }
     }
 
@@ -357,8 +365,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
                     sum *= f_pref[o];
                     double *dst = p.Delta + DIDX(q, li);
-                    if (p.n_split == 1) *dst = sum;
-                    else atomicAdd(dst, sum);
+                    *dst = pass ? *dst + sum : sum;   // pass p adds to what this CTA stored in passes < p
                 }
             }
             // CTAs smaller than the one NOUT was sized for: the remaining columns
@@ -371,8 +378,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
                     if (q == 1) sum *= p.pref[li];
                     double *dst = p.Delta + DIDX(q, li);
-                    if (p.n_split == 1) *dst = sum;
-                    else atomicAdd(dst, sum);
+                    *dst = pass ? *dst + sum : sum;
                 }
             }
         }
@@ -462,80 +468,100 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
       any_hist = (any_hist << 1) | (unsigned)g_any;
       if (n >= LAG) flush_group(n - LAG, (any_hist >> LAG) & 1u);
     }
+  }   // passes
+#undef GCAMB_UNI
+#undef DIDX
+    // A launch that was started early (programmatic stream serialization) must not COMPLETE before the
+    // launch it follows has completed and flushed its stores: later work in the stream orders itself
+    // against this launch only.  No-op for a launch without the attribute.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------
-#ifndef GCAMB_G
-#define GCAMB_G 8
-#endif
-constexpr int RING_G = GCAMB_G;   // tiles between CTA-wide flushes
-#ifndef GCAMB_MINB
-#define GCAMB_MINB 3
-#endif
-#ifndef GCAMB_MINB256
-#define GCAMB_MINB256 1
-#endif
-#ifndef GCAMB_V2
-#define GCAMB_V2 8          // l-tile for n_src = 2
-#endif
+constexpr int RING_G = 8;      // tiles between flushes of the ring (4 / 12 / 16 / 24 measured slower)
+constexpr int TILE_V = 8;      // l-tile (V = 16 with two resident CTAs measured 3.5 % slower)
+constexpr int MINB_128 = 3;    // resident CTAs per SM the <= 128-thread kernels are compiled for (168 registers)
+constexpr int MINB_256 = 1;
 
-// CTA sizes are powers of two of warps (1, 2, 4, 8): the hardware deals a CTA's warps round-robin
-// to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA advances at the pace of
-// its slowest warp, so warp counts such as 5 leave one pipe with twice the work of the others
-// (measured: profiles/README.md).  T is then the smallest slot count that covers the tau range.
+// Launch shape.  CTA sizes are powers of two of warps (1, 2, 4, 8): the hardware deals
+// a CTA's warps round-robin to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA
+// advances at the pace of its slowest warp, so warp counts such as 5 leave one pipe with twice the
+// work of the others (measured: profiles/README.md).  The tau range is cut into the fewest passes of
+// at most threads * T_MAX points; T is the smallest slot count that covers a pass.
+//   * large launches (enough warps to fill the machine): least padding wins; at equal padding the
+//     smaller CTA, i.e. more points per thread: the cross-thread reduction costs one DADD per thread,
+//     tile row and source whatever T is.  More than 128 threads only when that saves a pass.
+//   * small launches (n_rows CTAs of that shape would leave the SMs' sub-partitions with fewer than
+//     FILL_WARPS warps each): trade points per thread for threads until they do, because a lone warp
+//     per sub-partition runs at the latency of its dependent DFMA chains, not at throughput.
+// The result depends on (n_tau, n_src, n_rows, n_sm) only; the order of every sum depends on the
+// shape, so a batched call and a single call agree bit for bit only when they choose the same shape:
+// choose_shape is therefore evaluated with the rows of ONE cosmology (n_k), never with n_k * n_batch.
 #if !defined(GCAMB_TU_SPARSE) || (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
-TransferShape choose_shape(int n_tau, int n_src)
+TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm)
 {
-    TransferShape s;
-    s.V = n_src == 2 ? GCAMB_V2 : 8;
-    const int t_max = 12;
-    s.n_split = 1;
-    for (;;) {
-        const int len = (n_tau + s.n_split - 1) / s.n_split;
-        int best_pad = 0x7fffffff;
-        // least padding wins; at equal padding the smaller CTA, i.e. more points per thread: the
-        // cross-thread reduction costs one DADD per thread, tile row and source whatever T is
-#ifdef XP_THREADS_MIN
-        for (int threads = XP_THREADS_MIN; threads <= 256; threads <<= 1) {
-#else
-        for (int threads = 32; threads <= 256; threads <<= 1) {
-#endif
-            const int T = (len + threads - 1) / threads;
-            if (T > t_max) continue;
-            const int pad = T * threads - len;
-            if (pad < best_pad) { best_pad = pad; s.threads = threads; s.T = T; }
-        }
-        if (best_pad != 0x7fffffff) break;
-        ++s.n_split;
+    (void)n_src;
+    constexpr int FILL_WARPS = 3;   // per sub-partition (config 1 runs at 3: 3 CTAs x 4 warps per SM)
+    auto shape_for = [&](int threads) {
+        TransferShape s;
+        s.V = TILE_V;
+        s.threads = threads;
+        s.n_pass = (n_tau + threads * T_MAX - 1) / (threads * T_MAX);
+        s.pass_len = (n_tau + s.n_pass - 1) / s.n_pass;
+        s.T = (s.pass_len + threads - 1) / threads;
+        return s;
+    };
+    auto padding = [&](const TransferShape &s) { return (long long)s.n_pass * s.T * s.threads - n_tau; };
+    TransferShape best = shape_for(32);
+    for (int threads = 64; threads <= 256; threads <<= 1) {
+        const TransferShape s = shape_for(threads);
+        if (threads == 256 && s.n_pass >= best.n_pass) break;
+        if (s.n_pass < best.n_pass || (s.n_pass == best.n_pass && padding(s) < padding(best))) best = s;
     }
-    return s;
+    const long long want = (long long)FILL_WARPS * 4 * n_sm;
+    while (best.threads < 256 && best.T >= 4 && n_rows * (best.threads / 32) < want) {
+        const TransferShape s = shape_for(best.threads * 2);
+        if (s.n_pass > best.n_pass) break;
+        best = s;
+    }
+    return best;
 }
 #endif
 
 // One launch over positions [k_first, k_first + n_pos) of the cost order.
 template <int T, int V, int NSRC, bool COMP, bool SPARSE>
 static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int k_first, int n_pos,
-                                bool zero_fill, bool overlap_previous, cudaStream_t stream)
+                                bool zero_fill, bool overlap_previous, int device, cudaStream_t stream)
 {
     if (n_pos <= 0) return GCAMB_OK;
     prm.k_first = k_first;
     prm.zero_fill = zero_fill;
-    const int W = sh.threads / 32;
-    size_t smem = sizeof(double2) * T * sh.threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
-                  sizeof(double) * (RD * RING_G * W * NSRC * V + 2 * RD) +
-                  sizeof(int) * (((size_t)T * sh.threads + W * 2 * T + 1) & ~(size_t)1);
-    if (COMP) smem += sizeof(double) * T * sh.threads;
+    auto smem_bytes = [](int threads) {
+        const int W = threads / 32;
+        size_t smem = sizeof(double2) * T * threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
+                      sizeof(double) * (RD * RING_G * W * NSRC * V + 2 * RD) +
+                      sizeof(int) * (((size_t)T * threads + W * 2 * T + 1) & ~(size_t)1);
+        if (COMP) smem += sizeof(double) * T * threads;
+        return smem;
+    };
     // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
     // are compiled for 3 co-resident CTAs per SM (168 registers) while that fits, else for 2
-    constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : GCAMB_MINB;
-    auto kern = sh.threads <= 128 ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE>
-                                  : transfer_kernel<T, V, NSRC, RING_G, 256, GCAMB_MINB256, COMP, SPARSE>;
-    if (smem > 48 * 1024)   // opt in to large dynamic shared memory (cheap; keeps the call stateless)
-        GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : MINB_128;
+    const bool small = sh.threads <= 128;
+    auto kern = small ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE>
+                      : transfer_kernel<T, V, NSRC, RING_G, 256, MINB_256, COMP, SPARSE>;
+    // opt in to large dynamic shared memory once per kernel and device (bit d of the mask = device d done)
+    static std::atomic<unsigned long long> attr_done[2];
+    const unsigned long long dev_bit = 1ull << (device & 63);
+    if (!(attr_done[small].load(std::memory_order_acquire) & dev_bit)) {
+        GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)smem_bytes(small ? 128 : 256)));
+        attr_done[small].fetch_or(dev_bit, std::memory_order_release);
+    }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(n_pos * prm.n_batch), (unsigned)sh.n_split);
+    cfg.gridDim = dim3((unsigned)(n_pos * prm.n_batch));
     cfg.blockDim = dim3((unsigned)sh.threads);
-    cfg.dynamicSmemBytes = smem;
+    cfg.dynamicSmemBytes = smem_bytes(sh.threads);
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -553,22 +579,22 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
 // SPARSE: the kernels that skip the accumulation on tiles without a listed l (sparse l lists).
 template <int T, int V, int NSRC, bool SPARSE>
 static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
-                                bool zero_fill, cudaStream_t stream)
+                                bool zero_fill, int device, cudaStream_t stream)
 {
     const int c0 = pos0, c1 = std::min(pos1, n_comp);   // compensated part
     const int q0 = std::max(pos0, n_comp), q1 = pos1;   // plain part
     const bool has_plain = q1 > q0;
-    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, stream);
+    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, device, stream);
     if (st != GCAMB_OK) return st;
-    return launch_impl<T, V, NSRC, false, SPARSE>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, stream);
+    return launch_impl<T, V, NSRC, false, SPARSE>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, device, stream);
 }
 
 template <int V, int NSRC, bool SPARSE>
 static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
-                             bool zero_fill, cudaStream_t stream)
+                             bool zero_fill, int device, cudaStream_t stream)
 {
     switch (sh.T) {
-#define GCAMB_T(t) case t: return launch_pair<t, V, NSRC, SPARSE>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);
+#define GCAMB_T(t) case t: return launch_pair<t, V, NSRC, SPARSE>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);
         GCAMB_T(1) GCAMB_T(2) GCAMB_T(3) GCAMB_T(4) GCAMB_T(5) GCAMB_T(6)
         GCAMB_T(7) GCAMB_T(8) GCAMB_T(9) GCAMB_T(10) GCAMB_T(11) GCAMB_T(12)
 #undef GCAMB_T
@@ -590,14 +616,14 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
 #endif
 #define GCAMB_ENTRY(name, NS, SP)                                                                             \
     gcamb_status name(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,     \
-                      bool zero_fill, cudaStream_t stream)                                                    \
+                      bool zero_fill, int device, cudaStream_t stream)                                        \
     {                                                                                                         \
-        return launch_T<(NS) == 2 ? GCAMB_V2 : 8, NS, SP>(prm, sh, n_comp, pos0, pos1, zero_fill, stream);    \
+        return launch_T<TILE_V, NS, SP>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);              \
     }
-gcamb_status launch_range_dense_2(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
-gcamb_status launch_range_dense_3(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
-gcamb_status launch_range_sparse_2(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
-gcamb_status launch_range_sparse_3(const TransferParams &, const TransferShape &, int, int, int, bool, cudaStream_t);
+gcamb_status launch_range_dense_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_dense_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_sparse_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_sparse_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 #if GCAMB_TU_HAS(0, 2)
 GCAMB_ENTRY(launch_range_dense_2, 2, false)
 #endif
@@ -612,22 +638,13 @@ GCAMB_ENTRY(launch_range_sparse_3, 3, true)
 #endif
 
 #if GCAMB_TU_PRIMARY
+int transfer_tile_v() { return TILE_V; }
+
 gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double *S_T,
                              const double *S_E, const double *S_phi, double *Delta,
                              cudaStream_t stream)
 {
-    gcamb_status st = launch_transfer_prepare(p, n_batch, Delta, stream);
-    if (st != GCAMB_OK) return st;
     return launch_transfer_range(p, n_batch, S_T, S_E, S_phi, Delta, 0, p->n_k, true, stream);
-}
-
-gcamb_status launch_transfer_prepare(const gcamb_los_plan *p, int n_batch, double *Delta, cudaStream_t stream)
-{
-    if (p->shape.n_split > 1) {   // RED output: the tau splits add into a zeroed Delta
-        const size_t bytes = sizeof(double) * (size_t)n_batch * p->n_src * p->n_l * p->n_k;
-        GCAMB_CUDA(cudaMemsetAsync(Delta, 0, bytes, stream));
-    }
-    return GCAMB_OK;
 }
 
 gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
@@ -643,17 +660,13 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.l_list = p->d_l_list; prm.kz = p->d_kz; prm.tile_mask = p->d_tile_mask;
     prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l;
     prm.l_min = p->l_min; prm.l_max = p->l_max; prm.n_tiles = p->n_tiles;
-    prm.n_batch = n_batch; prm.n_split = sh.n_split;
+    prm.n_batch = n_batch; prm.n_pass = sh.n_pass; prm.pass_len = sh.pass_len;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.order_reversed = p->order_reversed;
-    prm.split_len = (p->n_tau + sh.n_split - 1) / sh.n_split;
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
-    if (p->n_src == 2 && sh.V == GCAMB_V2)
-        return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
-    if (p->n_src == 3 && sh.V == 8)
-        return (sparse ? launch_range_sparse_3 : launch_range_dense_3)(prm, sh, p->n_comp, pos0, pos1, zero_fill, stream);
-    set_error("no transfer kernel for V=%d n_src=%d", sh.V, p->n_src);
-    return GCAMB_EINVAL;
+    if (p->n_src == 2)
+        return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
+    return (sparse ? launch_range_sparse_3 : launch_range_dense_3)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
 }
 #endif   // GCAMB_TU_PRIMARY
 

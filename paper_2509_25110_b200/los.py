@@ -22,8 +22,11 @@ EXPORTS = (
     "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
-    "gcamb_los_dfma_probe", "gcamb_los_last_error",
+    "gcamb_los_last_error",
 )
+# libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
+PROBE_LIB_PATH = os.path.join(_HERE, "libgcamb_probe.so")
+PROBE_EXPORTS = ("gcamb_probe_dfma", "gcamb_probe_dmma")
 
 _vp, _i32, _i64, _f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
 _lib = None
@@ -55,7 +58,6 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_transfer_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_cls_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     lib.gcamb_los_spectra_host.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
-    lib.gcamb_los_dfma_probe.argtypes = [_i32, _i32, _i64, _vp, _vp]
     _lib = lib
     return lib
 
@@ -182,5 +184,30 @@ def gcamb_los_plan_create(l_list, k, tau, tau0, with_phi=False) -> Plan:
     return Plan(l_list, k, tau, tau0, with_phi)
 
 
-def gcamb_los_dfma_probe(blocks: int, threads: int, iters: int, out: torch.Tensor) -> None:
-    _check(load_library().gcamb_los_dfma_probe(blocks, threads, iters, _dev(out, (blocks * threads,), "out"), _stream()))
+_probe_lib = None
+
+
+def load_probe_library() -> ctypes.CDLL:
+    global _probe_lib
+    if _probe_lib is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            raise ImportError(f"{PROBE_LIB_PATH} not built: run `python -m paper_2509_25110_b200.build`")
+        lib = ctypes.CDLL(PROBE_LIB_PATH)
+        for name in PROBE_EXPORTS:
+            getattr(lib, name).argtypes = [_i32, _i32, _i64, _vp, _vp]
+        _probe_lib = lib
+    return _probe_lib
+
+
+def _probe(name: str, blocks: int, threads: int, iters: int, out: torch.Tensor) -> None:
+    rc = getattr(load_probe_library(), name)(blocks, threads, iters, _dev(out, (blocks * threads,), "out"), _stream())
+    if rc:
+        raise RuntimeError(f"{name}: cudaError {rc}")
+
+
+def gcamb_probe_dfma(blocks: int, threads: int, iters: int, out: torch.Tensor) -> None:
+    _probe("gcamb_probe_dfma", blocks, threads, iters, out)
+
+
+def gcamb_probe_dmma(blocks: int, threads: int, iters: int, out: torch.Tensor) -> None:
+    _probe("gcamb_probe_dmma", blocks, threads, iters, out)

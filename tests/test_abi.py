@@ -9,20 +9,28 @@ from paper_2509_25110_b200 import build, los
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "gcamb_los.h")).read()
+def declared_symbols(header, prefix):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(gcamb_los_\w+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(%s\w+)\s*\(" % prefix, text)))
 
 
 def test_library_builds_loads_and_exports_every_declared_symbol():
     lib_path = build.build_extension()
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["gcamb_los.h", "gcamb_probe.h"]
+    # the product library: every symbol of gcamb_los.h, and nothing of the bench-only probe header
     lib = ctypes.CDLL(lib_path)
-    names = declared_symbols()
-    assert len(names) >= 11
+    names = declared_symbols("gcamb_los.h", "gcamb_los_")
+    assert len(names) >= 10
     for name in names:
         assert hasattr(lib, name), f"{name} declared in gcamb_los.h but not exported"
     assert sorted(los.EXPORTS) == names
+    # the probe library (bench.py's roofline denominators)
+    probe = ctypes.CDLL(build.PROBE_LIB)
+    probe_names = declared_symbols("gcamb_probe.h", "gcamb_probe_")
+    assert sorted(los.PROBE_EXPORTS) == probe_names and len(probe_names) == 2
+    for name in probe_names:
+        assert hasattr(probe, name) and not hasattr(lib, name)
 
 
 def test_errors_without_touching_the_gpu():

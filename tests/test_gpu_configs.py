@@ -1,14 +1,16 @@
 """GPU parity at BASELINE.json's full config sizes, in the launch configuration bench.py times.
 
 Configs 1 and 2 are compared element by element with the long-double oracle (the whole Delta
-and C_l).  Config 3 runs all 64 cosmologies in one batched launch pair and compares three of
-them in full.  Config 4 is too large for the oracle to finish in seconds, so
+and C_l).  Config 3 runs all 64 cosmologies in one batched launch pair and compares sixteen of
+them in full.  Config 4 (4.8 GB of Delta) is compared with the oracle on EVERY k row, in ten
+sub-problems of every 10th k (offsets 0..9; same l range, same tau grid, hence the same CTA shape
+and the same per-k work):
   * the full-size run is checked on properties (every element written and finite, zero exactly
     where R16 says so, TT/EE/phiphi >= 0, Cauchy-Schwarz for TE),
-  * a sub-problem with every 10th k (same l range, same tau grid, hence the same CTA shape and
-    the same per-k work) is compared element by element with the oracle, Delta and C_l,
-  * and the rows the two GPU runs share must agree bit for bit (a k row never depends on the
-    other rows).
+  * each sub-problem's rows must equal the full run's rows bit for bit (a k row never depends on
+    the other rows) and are compared element by element with the long-double oracle; the per-l
+    error is then formed over all 20000 k rows (largest |difference| over all rows / largest
+    |Delta_l| over all rows), and the first sub-problem's C_l is compared too.
 Outputs are pre-filled with NaN so an element the kernels fail to write cannot pass.
 
 Bars as in test_gpu_parity.py: |dDelta| <= 1e-10 max_k|Delta_l| per (source, l); C_l 1e-8 (R13).
@@ -20,7 +22,10 @@ itself differs from the long-double build by up to 1.2e-10 there.  The tolerance
 silently: an l may exceed 1e-10 only where the fp64 oracle comes within a factor 2 of the same error
 (largest fp64-oracle error within 512 l: the errors are noise-like from one l to the next), the
 largest GPU error may not exceed 1.5 x the largest fp64-oracle error, and fewer than 1 % of the
-l may be over 1e-10 (measured: 12 l for the GPU path, 17 l for the fp64 oracle; both peak at 1.2e-10).
+l may be over 1e-10.  The fp64 oracle is run on every k row as well, so both error profiles are
+maxima over the same 20000 rows.  DESIGN.md 6.3 carries the measured counts, and those of the one
+variant tried against it (coefficient carried as hi + lo through the recurrence step: more l over
+the bar, not fewer, at +21 % time).
 """
 import numpy as np
 import pytest
@@ -121,7 +126,7 @@ def test_config3_emulator_batch(los):
     S_E = torch.empty_like(S_T)
     P = torch.empty(B, cfg.n_k, dtype=torch.float64, device="cuda")
     host = {}
-    check = (0, 17, 63)
+    check = tuple(range(0, 64, 4))          # 16 of the 64 cosmologies, element by element
     for c in range(B):
         s = synth.sources(cfg, c)
         S_T[c].copy_(torch.from_numpy(s[0]))
@@ -158,36 +163,44 @@ def test_config4_extreme(los):
     assert plan.nominal_terms == cfg.nominal_terms()
     assert bool(torch.isfinite(D).all())
     cl_properties(C.cpu().numpy())
-    rows = torch.arange(0, cfg.n_k, stride, device="cuda")
-    D_rows = D[:, :, rows].cpu().numpy()
-    del D, C, S
+    del C, S
     plan.close()
-    torch.cuda.empty_cache()
 
-    sl = slice(0, cfg.n_k, stride)
-    plan_s, k_s, S_s, P_s, D_s, C_s = run_single(los, cfg, sl)
-    D_s, C_s = D_s.cpu().numpy(), C_s.cpu().numpy()
-    assert np.array_equal(D_s, D_rows)          # a k row does not depend on the other rows
-    D_ref, C_ref = oracle_run(cfg, k_s, S_s, P_s)
-    D_f64 = oracle.transfer(cfg.l_list(), k_s, cfg.tau(), cfg.tau0, S_s[0], S_s[1], S_s[2], real="f64")
-    scale = np.max(np.abs(D_ref), axis=-1)
+    n_src, n_l = 3, cfg.n_l
+    err = np.zeros((n_src, n_l)); err64 = np.zeros((n_src, n_l)); scale = np.zeros((n_src, n_l))
+    for off in range(stride):
+        sl = slice(off, cfg.n_k, stride)
+        rows = torch.arange(off, cfg.n_k, stride, device="cuda")
+        plan_s, k_s, S_s, P_s, D_s, C_s = run_single(los, cfg, sl)
+        assert torch.equal(D_s, D[:, :, rows])          # a k row does not depend on the other rows
+        D_s = D_s.cpu().numpy()
+        D_ref, C_ref = oracle_run(cfg, k_s, S_s, P_s)
+        D_f64 = oracle.transfer(cfg.l_list(), k_s, cfg.tau(), cfg.tau0, S_s[0], S_s[1], S_s[2], real="f64")
+        err = np.maximum(err, np.max(np.abs(D_s - D_ref), axis=-1))
+        err64 = np.maximum(err64, np.max(np.abs(D_f64 - D_ref), axis=-1))
+        scale = np.maximum(scale, np.max(np.abs(D_ref), axis=-1))
+        assert np.all(D_s[D_ref == 0.0] == 0.0)
+        if off == 0:
+            e_auto, e_te = cl_err(C_s.cpu().numpy(), C_ref)
+            assert e_auto <= TOL_CL and e_te <= TOL_CL
+        plan_s.close()
+        del D_s, D_ref, D_f64, S_s
     scale = np.where(scale > 0, scale, 1.0)
-    e_gpu = np.max(np.abs(D_s - D_ref), axis=-1) / scale          # [source][l]
-    e_f64 = np.max(np.abs(D_f64 - D_ref), axis=-1) / scale        # the fp64 floor, same normaliser
+    e_gpu = err / scale            # [source][l], over all 20000 k rows
+    e_f64 = err64 / scale          # the fp64 floor, same rows, same normaliser
     win = 512
     pad = np.pad(e_f64, ((0, 0), (win, win)), mode="edge")
     floor = np.max(np.lib.stride_tricks.sliding_window_view(pad, 2 * win + 1, axis=1), axis=-1)
     over = e_gpu > TOL_DELTA
-    print(f"config 4: max Delta error {e_gpu.max():.3e}; l over 1e-10 per source: {over.sum(axis=1).tolist()}; "
-          f"fp64 oracle vs long double: max {e_f64.max():.3e}, l over 1e-10: {(e_f64 > TOL_DELTA).sum(axis=1).tolist()}")
+    print(f"config 4, all {cfg.n_k} k rows: max Delta error {e_gpu.max():.3e}; l over 1e-10 per source: "
+          f"{over.sum(axis=1).tolist()}; fp64 oracle vs long double: max {e_f64.max():.3e}, "
+          f"l over 1e-10: {(e_f64 > TOL_DELTA).sum(axis=1).tolist()}")
     assert np.all(e_gpu <= np.maximum(TOL_DELTA, 2.0 * floor)), "Delta error above 1e-10 and above twice the fp64 floor"
     assert e_gpu.max() <= max(TOL_DELTA, 1.5 * e_f64.max())
     assert np.all(e_gpu[2] <= TOL_DELTA)                          # the lensing source is not in that regime
     assert over.sum() < 0.01 * over.size
-    e_auto, e_te = cl_err(C_s, C_ref)
-    assert e_auto <= TOL_CL and e_te <= TOL_CL
-    assert np.all(D_s[D_ref == 0.0] == 0.0)
-    plan_s.close()
+    # below l = 7000 the plain bar holds with margin
+    assert np.all(e_gpu[:, : 7000 - cfg.l_min] <= 0.2 * TOL_DELTA)
 
 
 def test_config1_sparse_l_list_equals_the_dense_rows(los):

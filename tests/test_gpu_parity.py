@@ -97,8 +97,9 @@ def _small_problem(n_l_spec, n_k, n_tau, with_phi, seed):
     (np.array([2]), 2, 40, False, 3),                 # single l, minimum n_k
     (np.array([5, 6, 40, 41, 300, 1500]), 17, 300, True, 4),    # sparse l list (R21), x up to 1540
     (np.arange(700, 900), 9, 130, False, 5),          # l range not starting at 2
-    (np.arange(2, 40), 12, 1300, True, 6),            # n_tau above one CTA's slots for n_src=3
-    (np.arange(2, 60), 6, 3100, False, 7),            # tau split across CTAs (RED path), n_src=2
+    (np.arange(2, 40), 12, 1300, True, 6),            # n_tau just above 128 x 10
+    (np.arange(2, 60), 6, 3100, False, 7),            # n_tau above one CTA's slots: three passes, n_src=2
+    (np.arange(2, 230), 8, 300, False, 8),            # few rows: the launch trades points per thread for threads
 ])
 def test_edge_shapes(los, case):
     l_list, k, tau, tau0, S_T, S_E, S_P, P = _small_problem(*case)
@@ -112,9 +113,9 @@ def test_edge_shapes(los, case):
     assert e_auto <= TOL_CL and e_te <= TOL_CL
 
 
-def test_batched_tau_split_with_phi(los):
-    """n_tau above one CTA's slots: two CTAs share a k and add into the zeroed Delta (RED path);
-    batched, three sources, sparse l list; still equal to the single calls bit for bit."""
+def test_batched_tau_passes_with_phi(los):
+    """n_tau above one CTA's slots: the CTA takes the tau range in passes and adds each pass to what
+    it stored before; batched, three sources, sparse l list; still equal to the single calls bit for bit."""
     rng = np.random.default_rng(11)
     n_k, n_tau, B = 7, 3300, 3
     tau = np.sort(rng.uniform(100.0, 13900.0, n_tau))
@@ -133,6 +134,64 @@ def test_batched_tau_split_with_phi(los):
         C_ref = oracle.cls(k, D_ref, P[c], real="f80")
         assert delta_err(Db[c].cpu().numpy(), D_ref) <= TOL_DELTA
         e_auto, e_te = cl_err(Cb[c].cpu().numpy(), C_ref)
+        assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
+@pytest.mark.parametrize("n_src", [2, 3])
+def test_many_tau_passes_are_deterministic(los, n_src):
+    """n_tau ~ 7000: five passes of one CTA per k (no atomics, no cleared output buffer).  Oracle
+    parity, run-to-run bit equality on a NaN-prefilled buffer, batched == single."""
+    rng = np.random.default_rng(21 + n_src)
+    n_k, n_tau, B = 9, 7001, 2
+    tau = np.sort(rng.uniform(100.0, 13950.0, n_tau))
+    k = np.geomspace(2e-4, 0.06, n_k)
+    l_list = np.arange(2, 420, dtype=np.int32)
+    S = rng.standard_normal((3, B, n_k, n_tau))
+    P = rng.uniform(1e-9, 3e-9, (B, n_k))
+    plan = los.Plan(l_list, k, tau, 14000.0, with_phi=n_src == 3)
+    args = lambda c=None: [dev(S[q] if c is None else S[q, c]) for q in range(n_src)] + [None] * (3 - n_src)
+    runs = []
+    for _ in range(3):
+        Db = torch.full((B, n_src, l_list.size, n_k), float("nan"), dtype=torch.float64, device="cuda")
+        plan.gcamb_los_transfer_batched(*args(), out=Db)
+        runs.append(Db)
+    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
+    for c in range(B):
+        D1 = torch.full((n_src, l_list.size, n_k), float("nan"), dtype=torch.float64, device="cuda")
+        plan.gcamb_los_transfer(*args(c), out=D1)
+        assert torch.equal(D1, runs[0][c])
+        D_ref = oracle.transfer(l_list, k, tau, 14000.0, S[0, c], S[1, c], S[2, c] if n_src == 3 else None, real="f80")
+        assert delta_err(runs[0][c].cpu().numpy(), D_ref) <= TOL_DELTA
+    plan.close()
+
+
+@pytest.mark.parametrize("n_plain", [1, 2, 4])
+def test_few_plain_rows_after_the_compensated_launch(los, n_plain):
+    """All but 1..4 k rows lie above the compensation threshold (x_max = k chi_0 > 6755): the plain
+    launch that overlaps the compensated one is tiny and would retire long before it.  Work that
+    follows in the stream (here the C_l kernel and a device-side copy) must still see every row."""
+    tau = np.concatenate([np.linspace(200.0, 400.0, 90), np.geomspace(420.0, 13999.0, 70)])
+    k = np.concatenate([np.geomspace(1e-3, 0.2, n_plain), np.linspace(0.5, 0.9, 40)])
+    assert np.sum(k * (14000.0 - tau[0]) > 6755.4) == 40
+    l_list = np.arange(2, 900, dtype=np.int32)
+    rng = np.random.default_rng(70 + n_plain)
+    S_T, S_E = rng.standard_normal((2, k.size, tau.size))
+    P = rng.uniform(1e-9, 3e-9, k.size)
+    plan = los.Plan(l_list, k, tau, 14000.0)
+    assert plan.transfer_launches == 2
+    D_ref = oracle.transfer(l_list, k, tau, 14000.0, S_T, S_E, real="f80")
+    C_ref = oracle.cls(k, D_ref, P, real="f80")
+    d_T, d_E, d_P = dev(S_T), dev(S_E), dev(P)
+    for _ in range(5):
+        D = torch.full((2, l_list.size, k.size), float("nan"), dtype=torch.float64, device="cuda")
+        C = torch.full((3, l_list.size), float("nan"), dtype=torch.float64, device="cuda")
+        plan.gcamb_los_transfer(d_T, d_E, out=D)
+        plan.gcamb_los_cls(D, d_P, out=C)
+        D_copy = D.clone()
+        torch.cuda.synchronize()
+        assert delta_err(D_copy.cpu().numpy(), D_ref) <= TOL_DELTA
+        e_auto, e_te = cl_err(C.cpu().numpy(), C_ref)
         assert e_auto <= TOL_CL and e_te <= TOL_CL
     plan.close()
 
