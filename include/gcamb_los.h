@@ -136,6 +136,36 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
                                    void *cuda_stream);
 
 /*
+ * Batched sources -> spectra in one call, WITHOUT the transfer functions ever reaching memory
+ * (the emulator-training use-case: 1e5-1e6 spectra on a fixed grid; Eq. 1-3,
+ * PAPER.md:50-58).  For plans with the T and E sources only and n_tau <= 2560 this runs ONE fused
+ * kernel plus a small finishing kernel: x = k (tau0 - tau) does not depend on the cosmology, so the
+ * j_l recurrence is evaluated once per (l, k, tau) for a block of 8 (or 4) cosmologies, the tau-sum
+ * becomes a dense [l x tau] . [tau x (X, cosmology)] contraction on the FP64 tensor cores
+ * (mma.sync.m8n8k4.f64), and Eq. 1 is accumulated over k inside the kernel from per-thread-block
+ * partial spectra that are added in a fixed order: results are bit-reproducible run to run.  They
+ * are NOT bit-identical to gcamb_los_transfer_batched + gcamb_los_cls_batched (another summation
+ * order; both are within the tolerances of BJ).  Other plans (phi source, longer tau grids, sparse
+ * l lists) and n_batch = 1 take those two calls internally, with Delta in scratch of the plan.
+ *   d_S_T, d_S_E, d_S_phi DEVICE [n_batch][n_k][n_tau] (d_S_phi NULL iff the plan has no phi);
+ *   d_P_R DEVICE [n_batch][n_k];  d_Cl DEVICE [n_batch][n_spec][n_l], order TT, EE, TE, (phiphi).
+ * Asynchronous on `cuda_stream`.  Scratch (partial spectra: n_SM x ceil(n_batch/8) x 3 x n_l x 8
+ * doubles, or Delta) belongs to the plan, is allocated on first use and grows when a larger batch
+ * arrives (that call synchronises the device); NOT thread-safe per plan.
+ */
+gcamb_status gcamb_los_spectra_batched(gcamb_los_plan *plan, int32_t n_batch,
+                                       const double *d_S_T, const double *d_S_E, const double *d_S_phi,
+                                       const double *d_P_R, double *d_Cl, void *cuda_stream);
+
+/*
+ * What gcamb_los_spectra_batched does for this plan and batch size: *fused = 1 if the fused kernel
+ * applies, *kernels = kernels of this library one call launches, *scratch_bytes = plan scratch it
+ * needs.  Any output pointer may be NULL.
+ */
+gcamb_status gcamb_los_spectra_batched_info(const gcamb_los_plan *plan, int32_t n_batch, int32_t *fused,
+                                            int32_t *kernels, int64_t *scratch_bytes);
+
+/*
  * End-to-end call with HOST buffers (the paper's "accelerator data region"):
  * H2D of the sources and P_R, transfer, cls, D2H of C_l (and of Delta when h_Delta != NULL), then
  * synchronises `cuda_stream`.  The sources are copied in four blocks of k rows (heaviest rows first)

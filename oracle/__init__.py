@@ -55,6 +55,7 @@ def _lib(real: str) -> ctypes.CDLL:
                                             ctypes.c_double, _pd, _pd, _pd, ctypes.c_int, ctypes.c_int, _pd]
             lib.oracle_cls.argtypes = [ctypes.c_int, ctypes.c_int, _pd, ctypes.c_int, _pd, _pd,
                                        ctypes.c_int, _pd]
+            lib.oracle_cl_interp.argtypes = [_pi, ctypes.c_int, ctypes.c_int, _pd, _pd]
             assert lib.oracle_real_mant_bits() == (53 if real == "f64" else 64)
             _LIBS[real] = lib
         return _LIBS[real]
@@ -121,4 +122,18 @@ def cls(k, Delta, P_R, real: str = "f64", nthreads: int = 0) -> np.ndarray:
     rc = _lib(real).oracle_cls(n_src, n_l, _ptr(k), n_k, _ptr(Delta), _ptr(P_R), int(nthreads), _ptr(out))
     if rc:
         raise ValueError(f"oracle_cls failed ({rc})")
+    return out
+
+
+def cl_interp(l_list, Cl_samp, real: str = "f64") -> np.ndarray:
+    """C_l on every integer l from l_list[0] to l_list[-1] from C_l on the sparse list (reading R25:
+    natural cubic spline of l(l+1) C_l in l).  Cl_samp [n_spec][n_l] -> [n_spec][l_last - l_first + 1]."""
+    l_list = np.ascontiguousarray(l_list, dtype=np.int32)
+    Cl_samp = _f64(Cl_samp)
+    n_spec, n_l = Cl_samp.shape
+    assert n_l == l_list.size
+    out = np.empty((n_spec, int(l_list[-1] - l_list[0] + 1)), dtype=np.float64)
+    rc = _lib(real).oracle_cl_interp(l_list.ctypes.data_as(_pi), n_l, n_spec, _ptr(Cl_samp), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_cl_interp failed ({rc})")
     return out

@@ -52,6 +52,7 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
     cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile); cudaFree(p->d_inv);
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
+    cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     if (p->h_streams_ready) {
@@ -248,6 +249,46 @@ gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, co
                            double *d_Cl, void *cuda_stream)
 {
     return gcamb_los_cls_batched(plan, 1, d_Delta, d_P_R, d_Cl, cuda_stream);
+}
+
+gcamb_status gcamb_los_spectra_batched(gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,
+                                       const double *d_S_E, const double *d_S_phi, const double *d_P_R,
+                                       double *d_Cl, void *cuda_stream)
+{
+    gcamb_status st = check_call(plan, n_batch, d_S_T, d_S_E, d_S_phi, d_Cl);
+    if (st != GCAMB_OK) return st;
+    if (!d_P_R) { set_error("null P_R"); return GCAMB_EINVAL; }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const bool fused = fused_supported(plan, n_batch);
+    // scratch: the fused kernel's partial spectra, else the Delta of the two-kernel path
+    const size_t need = fused ? fused_scratch_bytes(plan, n_batch)
+                              : sizeof(double) * (size_t)n_batch * plan->n_src * plan->n_l * plan->n_k;
+    if (need > plan->fused_scratch_cap) {
+        // grow-only; a buffer still in use by earlier work on another stream must not be freed under it
+        GCAMB_CUDA(cudaDeviceSynchronize());
+        cudaFree(plan->d_fused_scratch);
+        plan->d_fused_scratch = nullptr;
+        plan->fused_scratch_cap = 0;
+        GCAMB_CUDA(cudaMalloc(&plan->d_fused_scratch, need));
+        plan->fused_scratch_cap = need;
+    }
+    if (fused) return launch_fused(plan, n_batch, d_S_T, d_S_E, d_P_R, plan->d_fused_scratch, d_Cl, s);
+    st = launch_transfer(plan, n_batch, d_S_T, d_S_E, d_S_phi, plan->d_fused_scratch, s);
+    if (st != GCAMB_OK) return st;
+    return launch_cls(plan, n_batch, plan->d_fused_scratch, d_P_R, d_Cl, s);
+}
+
+gcamb_status gcamb_los_spectra_batched_info(const gcamb_los_plan *plan, int32_t n_batch, int32_t *fused,
+                                            int32_t *kernels, int64_t *scratch_bytes)
+{
+    if (!plan || n_batch < 1) { set_error("null plan or n_batch < 1"); return GCAMB_EINVAL; }
+    const bool f = fused_supported(plan, n_batch);
+    if (fused) *fused = f;
+    if (kernels) *kernels = f ? 2 : (plan->n_comp > 0) + (plan->n_comp < plan->n_k) + 1;
+    if (scratch_bytes)
+        *scratch_bytes = (int64_t)(f ? fused_scratch_bytes(plan, n_batch)
+                                     : sizeof(double) * (size_t)n_batch * plan->n_src * plan->n_l * plan->n_k);
+    return GCAMB_OK;
 }
 
 }  // extern "C"

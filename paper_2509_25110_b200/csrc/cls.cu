@@ -9,13 +9,14 @@
 
 namespace gcamb {
 
-constexpr int CLS_THREADS = 256;
+constexpr int CLS_ROWS = 2;               // l rows per CTA (they share the weights)
+constexpr int CLS_THREADS_DEFAULT = 128;
 
 template <int VEC> struct Pack;
 template <> struct Pack<1> { double v[1]; };
 template <> struct alignas(16) Pack<2> { double v[2]; };
 
-template <int NSRC, int R, int VEC>
+template <int NSRC, int R, int VEC, int CLS_THREADS>
 __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restrict__ Delta,
                                                           const double *__restrict__ P_R,
                                                           const double *__restrict__ dlnk,
@@ -87,12 +88,12 @@ __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restri
     }
 }
 
-template <int NSRC, int R>
+template <int NSRC, int R, int THREADS>
 static void launch_rows(bool vec, dim3 grid, cudaStream_t stream, const double *Delta, const double *P_R,
                         const double *dlnk, double *Cl, int n_l, int n_k)
 {
-    if (vec) cls_kernel<NSRC, R, 2><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
-    else cls_kernel<NSRC, R, 1><<<grid, CLS_THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
+    if (vec) cls_kernel<NSRC, R, 2, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
+    else cls_kernel<NSRC, R, 1, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
 }
 
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,
@@ -100,13 +101,15 @@ gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delt
 {
     // 16-byte loads need even rows and aligned bases (every row then starts on a 16-byte boundary)
     const bool vec = p->n_k % 2 == 0 && ((uintptr_t)Delta | (uintptr_t)P_R) % 16 == 0;
-    // rows per CTA: 4 while that still leaves two CTAs per SM, else 2, else 1
-    int R = 4;
+    int R = CLS_ROWS, threads = CLS_THREADS_DEFAULT;
+    // few rows: one row per CTA keeps more SMs busy
     while (R > 1 && (long long)((p->n_l + R - 1) / R) * n_batch < 2LL * p->n_sm) R >>= 1;
     dim3 grid((unsigned)((p->n_l + R - 1) / R), (unsigned)n_batch);
-#define GCAMB_CLS(NS, RR) launch_rows<NS, RR>(vec, grid, stream, Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k)
-    if (p->n_src == 2) { if (R == 4) GCAMB_CLS(2, 4); else if (R == 2) GCAMB_CLS(2, 2); else GCAMB_CLS(2, 1); }
-    else               { if (R == 4) GCAMB_CLS(3, 4); else if (R == 2) GCAMB_CLS(3, 2); else GCAMB_CLS(3, 1); }
+#define GCAMB_CLS(NS, RR, TH) launch_rows<NS, RR, TH>(vec, grid, stream, Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k)
+#define GCAMB_CLS_R(NS, TH) do { if (R == 4) GCAMB_CLS(NS, 4, TH); else if (R == 2) GCAMB_CLS(NS, 2, TH); else GCAMB_CLS(NS, 1, TH); } while (0)
+    if (p->n_src == 2) { if (threads == 128) GCAMB_CLS_R(2, 128); else GCAMB_CLS_R(2, 256); }
+    else               { if (threads == 128) GCAMB_CLS_R(3, 128); else GCAMB_CLS_R(3, 256); }
+#undef GCAMB_CLS_R
 #undef GCAMB_CLS
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;

@@ -1,0 +1,390 @@
+// fused.cu -- sources of a BATCH of cosmologies -> C_l, in one kernel that never writes Delta
+// (the emulator use-case of PAPER.md:24, 248; Eq. 1-3).
+//
+// For the cosmologies of a batch x = k (tau0 - tau) is the same (one plan), so
+//   * the coefficient and the recurrence step  f_{l-1} = (2l+1)/x f_l - f_{l+1}  are issued ONCE
+//     per (l, k, tau) and shared by all cosmologies of a block of BC, and
+//   * the tau-sum  Delta^X_l(k; b) = sum_i j_l(x_i) s_X(b; tau_i)  IS a dense contraction
+//     [l-tile x tau] . [tau x (X, b)]: it runs on the FP64 tensor cores (mma.sync.m8n8k4.f64, DMMA).
+//     On B200 DMMA has the SAME peak as DFMA (measured: both 64 FMA/clk/SM, and mixed streams add
+//     up to one pipe's worth: profiles/README.md), so the gain is not a second pipe but (a) one
+//     issue slot per 256 FMAs instead of 8 two-cycle DFMA issues with their register-operand
+//     stalls, (b) the cross-lane (tau) reduction happens inside the MMA: no transposing warp
+//     reduction, and (c) 2 + 2 BC FP64 lane-slots per (l, k, tau) for BC cosmologies instead of 4 BC.
+//
+// Mapping: one CTA of 8 warps takes a k row and BC = 4 NB cosmologies; thread = T (k, tau) points
+// as in transfer.cu (lanes <-> 32 consecutive tau of a warp slot), recurrence state in registers.
+// Per l-tile (V = 8) and started slot a thread runs its 8 recurrence steps and writes j_l .. j_{l-7}
+// to a per-warp shared-memory tile [8][32 tau]; the warp reads it back as four A-fragment pairs
+// (rows = l, columns = 4 tau) and multiplies them with the B fragments it holds in registers for
+// the whole walk: the pre-weighted sources s_X(b; tau) of its own 32 tau, columns (b, X).  The D
+// fragments (8 l x 8 columns each) accumulate over the slots of the warp; the eight warps' tiles
+// meet in the ring of transfer.cu (mbarrier-paced, flushed one group late).
+//
+// Eq. 1 is folded into the flush: a thread owns one (l, b) of the group, sums the warps in fixed
+// order, applies the Delta^E prefactor and adds  w_b(k) Delta^X Delta^Y  to the CTA's own slice of
+// partial spectra in global memory (L2-resident, plain load/add/store: the CTA is the only writer).
+// A CTA walks a STATIC list of k rows (balanced by cost at plan creation), so the order of every sum
+// is fixed: results are bit-reproducible.  A last small kernel adds the slices in bin order and
+// multiplies by 4 pi.
+#include <algorithm>
+#include <atomic>
+
+#include "los_internal.cuh"
+#include "mbar.cuh"
+
+namespace gcamb {
+
+namespace {
+
+struct FusedParams {
+    const double *S_T, *S_E;   // [B][n_k][n_tau]
+    const double *P_R;         // [B][n_k]
+    double *Cpart;             // [n_cblk][n_bins][3][n_l][BC]
+    const double *k, *chi, *w, *pref, *inv_x, *dlnk;
+    const double2 *start;
+    const int32_t *tile, *l_index, *bin_start, *bin_items;
+    int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_bins, l_contig;
+};
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int NEVER = 0x7fffffff;
+constexpr int F_V = 8;          // l-tile = rows of an MMA
+constexpr int F_W = 8;          // warps per CTA
+constexpr int F_THREADS = 32 * F_W;
+constexpr int F_G = 4;          // tiles per ring group: G * V * BC (l, b) pairs = one per thread at BC = 8
+constexpr int F_RD = 3;         // ring stages
+constexpr int F_LAG = 1;
+constexpr int F_JS = 40;        // row stride of the j_l tile: 16-byte fragment loads of a quarter-warp hit 32 distinct banks
+
+__device__ __forceinline__ void dmma(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+
+template <int NB, int T> constexpr size_t fused_smem_bytes()
+{
+    constexpr int P = F_V * 8 * NB;
+    return sizeof(double2) * T * F_THREADS                       // start pairs
+         + sizeof(double) * 2 * T * F_THREADS                    // 1/x and its rounding residual
+         + sizeof(double) * F_W * 2 * F_V * F_JS                 // j_l tiles, double-buffered per warp
+         + sizeof(double) * (F_RD * F_G * F_W * P + 2 * F_RD)    // ring + its barriers
+         + sizeof(int) * (T * F_THREADS + F_W * 2 * T);          // start tiles, slot windows
+}
+
+// NB = 8-column blocks of the contraction: BC = 4 NB cosmologies x (T, E).  T = points per thread.
+template <int NB, int T>
+__global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p)
+{
+    constexpr int V = F_V, W = F_W, G = F_G, RD = F_RD, LAG = F_LAG, JS = F_JS;
+    constexpr int BC = 4 * NB;
+    constexpr int P = V * 2 * BC;        // ring entries per warp and tile: [row][b][X]
+    constexpr int NPAIR = G * V * BC;    // (l, b) pairs per group
+    static_assert(NPAIR <= F_THREADS, "one (l, b) pair per thread at the flush");
+    extern __shared__ double2 smem2[];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __reduce_min_sync(FULL, tid >> 5);
+    double2 *my_start = smem2 + tid;                                  // [j * THREADS]
+    double *base = reinterpret_cast<double *>(smem2 + (size_t)T * F_THREADS);
+    double *my_ix = base + tid;                                       // [j * THREADS]
+    double *my_ixlo = base + (size_t)T * F_THREADS + tid;
+    base += 2 * (size_t)T * F_THREADS;
+    double *jt = base + (size_t)warp * 2 * V * JS;                    // [2][V][JS]
+    base += (size_t)W * 2 * V * JS;
+    double *ring = base;                                              // [RD][G][W][P]
+    base += (size_t)RD * G * W * P;
+    const uint32_t bar_full = (uint32_t)__cvta_generic_to_shared(base);
+    const uint32_t bar_empty = bar_full + 8 * RD;
+    int *my_tile = reinterpret_cast<int *>(base + 2 * RD) + tid;      // [j * THREADS]
+    int *slot_win = reinterpret_cast<int *>(base + 2 * RD) + (size_t)T * F_THREADS + warp * 2 * T;
+
+    const int bin = blockIdx.x, cb = blockIdx.y, b0 = cb * BC;
+    double *cpart = p.Cpart + ((size_t)cb * p.n_bins + bin) * 3 * p.n_l * BC;   // this CTA's partial spectra [3][n_l][BC]
+    for (size_t i = tid; i < (size_t)3 * p.n_l * BC; i += F_THREADS) cpart[i] = 0.0;
+    if (tid == 0) for (int d = 0; d < 2 * RD; ++d) mbar_init(bar_full + 8 * d, W);
+    __syncthreads();
+
+    // flush: this thread's (tile of the group, row, cosmology)
+    const bool f_on = tid < NPAIR;
+    const int f_gi = tid / (V * BC), f_r = (tid / BC) % V, f_b = tid % BC;
+    // fragment coordinates
+    const int fr = lane >> 2, fc = lane & 3;
+    const int it0 = p.bin_start[bin], it1 = p.bin_start[bin + 1];
+
+  for (int it = it0; it < it1; ++it) {
+    if (it > it0) {   // the ring starts afresh; the partial spectra the other threads stored are visible
+        __syncthreads();
+        if (tid == 0)
+            for (int d = 0; d < 2 * RD; ++d) { mbar_inval(bar_full + 8 * d); mbar_init(bar_full + 8 * d, W); }
+        __syncthreads();
+    }
+    const int kidx = __reduce_min_sync(FULL, p.bin_items[it]);
+    const double kval = p.k[kidx];
+    const size_t row = (size_t)kidx * p.n_tau;
+    // Eq. 1 weight of this k for the flush thread's cosmology
+    double f_wk = 0.0;
+    if (f_on && b0 + f_b < p.n_batch) f_wk = p.dlnk[kidx] * p.P_R[(size_t)(b0 + f_b) * p.n_k + kidx];
+    const int t_begin_load = p.tile[row];   // start tile of the largest x
+
+    // ---- prologue: recurrence state of this thread's points, B fragments of this warp's slots
+    double fa[T], fb[T], Bf[T][8][NB];
+    int tp[T];
+#pragma unroll
+    for (int j = 0; j < T; ++j) {
+        const int sb = j * F_THREADS + ((warp + j) % W) * 32;   // first tau of this warp's slot j
+        const int i = sb + lane;
+        const bool valid = i < p.n_tau;
+        const int ic = valid ? i : p.n_tau - 1;
+        const double inv = p.inv_x[row + ic];
+        const double x = __dmul_rn(kval, p.chi[ic]);
+        const double res = fma(inv, x, -1.0);               // 1/x = inv + inv_lo, inv_lo = -inv (inv x - 1)
+        my_ix[j * F_THREADS] = valid ? inv : 0.0;
+        my_ixlo[j * F_THREADS] = valid ? -inv * res : 0.0;
+        tp[j] = valid ? p.tile[row + ic] : NEVER;
+        my_tile[j * F_THREADS] = tp[j];
+        my_start[j * F_THREADS] = p.start[row + ic];
+        fa[j] = fb[j] = 0.0;
+        // B fragment of MMA m: row (tau) = sb + 8 (m >> 1) + 2 fc + (m & 1), column = 8 nb + fr = (b, X)
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const int i2 = sb + 8 * (m >> 1) + 2 * fc + (m & 1);
+            const bool v2 = i2 < p.n_tau;
+            const int ic2 = v2 ? i2 : p.n_tau - 1;
+            const double w2 = v2 ? p.w[ic2] : 0.0;
+            const double inv2 = p.inv_x[row + ic2];
+            const double wx[2] = {w2, w2 * (inv2 * inv2)};   // s_T = w S_T, s_E = w S_E / x^2
+#pragma unroll
+            for (int nb = 0; nb < NB; ++nb) {
+                const int col = 8 * nb + fr, bl = col >> 1, X = col & 1;
+                const bool vb = b0 + bl < p.n_batch;
+                const int bc = vb ? b0 + bl : p.n_batch - 1;
+                const double *S = X ? p.S_E : p.S_T;
+                const double v = S[((size_t)bc * p.n_k + kidx) * p.n_tau + ic2];
+                Bf[j][m][nb] = vb ? wx[X] * v : 0.0;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < T; ++j) {
+        const int first = __reduce_min_sync(FULL, tp[j]);
+        const int last = __reduce_max_sync(FULL, tp[j] == NEVER ? -1 : tp[j]);
+        if (lane == 0) { slot_win[2 * j] = first; slot_win[2 * j + 1] = last; }
+    }
+    __syncwarp();
+    const int t_begin = __reduce_min_sync(FULL, t_begin_load);
+    const int n_walk = p.n_tiles - t_begin;
+
+    // flush of group m: warps summed in index order, Delta^E prefactor, Eq. 1 products into the partial spectra
+    auto flush_group = [&](int m) {
+        const int stage = m % RD;
+        const int gcount = min(G, n_walk - m * G);
+        mbar_wait(bar_full + 8 * stage, (m / RD) & 1);
+        if (f_on && f_gi < gcount) {
+            const int l = p.l_max - (t_begin + m * G + f_gi) * V - f_r;
+            const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
+            if (li >= 0) {
+                const double2 *e = reinterpret_cast<const double2 *>(
+                    ring + ((size_t)(stage * G + f_gi) * W) * P + (f_r * BC + f_b) * 2);
+                double dT = 0.0, dE = 0.0;
+#pragma unroll
+                for (int wv = 0; wv < W; ++wv) {
+                    const double2 v = e[(size_t)wv * (P / 2)];
+                    dT += v.x;
+                    dE += v.y;
+                }
+                dE *= p.pref[li];
+                const double wT = f_wk * dT, wE = f_wk * dE;
+                double *c = cpart + (size_t)li * BC + f_b;
+                const size_t sp = (size_t)p.n_l * BC;
+                c[0] = fma(wT, dT, c[0]);
+                c[sp] = fma(wE, dE, c[sp]);
+                c[2 * sp] = fma(wT, dE, c[2 * sp]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * stage);
+    };
+
+#define GCAMB_UNI(v) __reduce_min_sync(FULL, (v))
+    int na = 0;
+    int next_slot = GCAMB_UNI(slot_win[0]);
+    int inj = 0, inj_from = next_slot;
+    int buf = 0;
+    double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);
+    const int n_groups = (n_walk + G - 1) / G;
+    int t = t_begin;
+    for (int n = 0; n < n_groups + LAG; ++n) {
+      if (n < n_groups) {
+        if (n >= RD) mbar_wait(bar_empty + 8 * (n % RD), ((n / RD) - 1) & 1);
+        const int gcount = min(G, n_walk - n * G);
+        for (int g = 0; g < gcount; ++g, ++t, tl0 -= 2.0 * V) {
+            while (next_slot <= t) {
+                ++na;
+                next_slot = na < T ? GCAMB_UNI(slot_win[2 * na]) : NEVER;
+            }
+            if (inj_from <= t) {
+#pragma unroll
+                for (int j = 0; j < T; ++j) {
+                    if (my_tile[j * F_THREADS] == t) {
+                        const double2 st = my_start[j * F_THREADS];
+                        fa[j] = st.x;
+                        fb[j] = st.y;
+                    }
+                }
+                while (inj < T && GCAMB_UNI(slot_win[2 * inj + 1]) <= t) ++inj;
+                inj_from = inj < T ? GCAMB_UNI(slot_win[2 * inj]) : NEVER;
+            }
+            double2 *rb = reinterpret_cast<double2 *>(ring + ((size_t)((n % RD) * G + g) * W + warp) * P);
+            if (na > 0) {
+                double D[2][NB][2];   // even / odd MMAs accumulate apart: 2 NB independent chains
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) D[h][nb][0] = D[h][nb][1] = 0.0;
+#pragma unroll
+                for (int j = 0; j < T; ++j) {
+                    if (j < na) {
+                        // a2: eight steps of the recurrence; j_l, .., j_{l-7} of this lane's tau go to the tile
+                        const double ixj = my_ix[j * F_THREADS];
+                        const double e = tl0 * my_ixlo[j * F_THREADS];
+                        double *tile_w = jt + (size_t)buf * V * JS + lane;
+#pragma unroll
+                        for (int s = 0; s < V; ++s) {
+                            const double tl = tl0 - 2.0 * s;
+                            const double c = fma(tl, ixj, e);        // correctly rounded (2l+1)/x
+                            tile_w[s * JS] = fb[j];
+                            const double fn = fma(c, fb[j], -fa[j]);
+                            fa[j] = fb[j];
+                            fb[j] = fn;
+                        }
+                        __syncwarp();
+                        // a3: A fragments (row = l-row fr, column = tau 8 mm + 2 fc + {0,1}) x B fragments
+                        const double2 *tile_r = reinterpret_cast<const double2 *>(jt + (size_t)buf * V * JS + fr * JS + 2 * fc);
+#pragma unroll
+                        for (int mm = 0; mm < 4; ++mm) {
+                            const double2 a = tile_r[4 * mm];
+#pragma unroll
+                            for (int nb = 0; nb < NB; ++nb) {
+                                dmma(D[0][nb], a.x, Bf[j][2 * mm][nb]);
+                                dmma(D[1][nb], a.y, Bf[j][2 * mm + 1][nb]);
+                            }
+                        }
+                        buf ^= 1;   // the next slot writes the other tile: two tiles suffice (see __syncwarp above)
+                    }
+                }
+                // D fragment: row fr, columns 2 fc, 2 fc + 1 of block nb = (T, E) of cosmology 4 nb + fc
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb)
+                    rb[fr * BC + 4 * nb + fc] = make_double2(D[0][nb][0] + D[1][nb][0], D[0][nb][1] + D[1][nb][1]);
+            } else {
+                for (int idx = lane; idx < P / 2; idx += 32) rb[idx] = make_double2(0.0, 0.0);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_full + 8 * (n % RD));
+      }
+      if (n >= LAG) flush_group(n - LAG);
+    }
+#undef GCAMB_UNI
+  }   // k rows of this bin
+}
+
+// C_l[b][XY][l] = 4 pi sum over bins (in bin order) of the partial spectra
+__global__ void __launch_bounds__(256) fused_finish_kernel(const double *__restrict__ Cpart, double *__restrict__ Cl,
+                                                           int n_bins, int n_l, int n_batch, int BC)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int cb = blockIdx.y;
+    const size_t slice = (size_t)3 * n_l * BC;
+    if (idx >= slice) return;
+    const int bl = (int)(idx % BC);
+    const int li = (int)((idx / BC) % n_l);
+    const int spec = (int)(idx / ((size_t)BC * n_l));
+    const int b = cb * BC + bl;
+    if (b >= n_batch) return;
+    const double *src = Cpart + (size_t)cb * n_bins * slice + idx;
+    double s = 0.0;
+    for (int bin = 0; bin < n_bins; ++bin) s += src[(size_t)bin * slice];
+    Cl[((size_t)b * 3 + spec) * n_l + li] = 4.0 * 3.14159265358979323846 * s;
+}
+
+template <int NB, int T>
+gcamb_status launch_one(const FusedParams &prm, int n_cblk, int device, cudaStream_t stream)
+{
+    constexpr size_t smem = fused_smem_bytes<NB, T>();
+    static_assert(smem <= 227 * 1024, "shared memory of the fused kernel");
+    static std::atomic<unsigned long long> attr_done;
+    const unsigned long long dev_bit = 1ull << (device & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
+        GCAMB_CUDA(cudaFuncSetAttribute(fused_kernel<NB, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done.fetch_or(dev_bit, std::memory_order_release);
+    }
+    fused_kernel<NB, T><<<dim3((unsigned)prm.n_bins, (unsigned)n_cblk), F_THREADS, smem, stream>>>(prm);
+    GCAMB_CUDA(cudaGetLastError());
+    return GCAMB_OK;
+}
+
+}  // namespace
+
+// Largest n_tau the fused kernel holds in registers for a block of 8 (NB = 2) / 4 (NB = 1) cosmologies
+constexpr int FUSED_T_MAX_NB2 = 5, FUSED_T_MAX_NB1 = 10;
+
+bool fused_supported(const gcamb_los_plan *p, int n_batch)
+{
+    return p->n_src == 2 && n_batch >= 2 && p->n_tau <= F_THREADS * FUSED_T_MAX_NB1 && p->d_tile_mask == nullptr;
+}
+
+int fused_block(const gcamb_los_plan *p, int n_batch)
+{
+    return (n_batch > 4 && p->n_tau <= F_THREADS * FUSED_T_MAX_NB2) ? 8 : 4;
+}
+
+size_t fused_scratch_bytes(const gcamb_los_plan *p, int n_batch)
+{
+    const int BC = fused_block(p, n_batch), n_cblk = (n_batch + BC - 1) / BC;
+    return sizeof(double) * (size_t)n_cblk * p->n_bins * 3 * p->n_l * BC;
+}
+
+gcamb_status launch_fused(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
+                          const double *P_R, double *scratch, double *Cl, cudaStream_t stream)
+{
+    FusedParams prm;
+    prm.S_T = S_T; prm.S_E = S_E; prm.P_R = P_R; prm.Cpart = scratch;
+    prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref; prm.inv_x = p->d_inv; prm.dlnk = p->d_dlnk;
+    prm.start = p->d_start; prm.tile = p->d_tile; prm.l_index = p->d_l_index;
+    prm.bin_start = p->d_bin_start; prm.bin_items = p->d_bin_items;
+    prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l; prm.l_min = p->l_min; prm.l_max = p->l_max;
+    prm.n_tiles = p->n_tiles; prm.n_batch = n_batch; prm.n_bins = p->n_bins;
+    prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
+    const int BC = fused_block(p, n_batch), n_cblk = (n_batch + BC - 1) / BC;
+    const int T = (p->n_tau + F_THREADS - 1) / F_THREADS;
+    gcamb_status st = GCAMB_EINVAL;
+    if (BC == 8) {
+        switch (T) {
+            case 1: st = launch_one<2, 1>(prm, n_cblk, p->device, stream); break;
+            case 2: st = launch_one<2, 2>(prm, n_cblk, p->device, stream); break;
+            case 3: st = launch_one<2, 3>(prm, n_cblk, p->device, stream); break;
+            case 4: st = launch_one<2, 4>(prm, n_cblk, p->device, stream); break;
+            case 5: st = launch_one<2, 5>(prm, n_cblk, p->device, stream); break;
+            default: set_error("fused kernel: n_tau %d too large for a block of 8", p->n_tau); return GCAMB_EINVAL;
+        }
+    } else {
+        switch ((T + 1) / 2) {
+            case 1: st = launch_one<1, 2>(prm, n_cblk, p->device, stream); break;
+            case 2: st = launch_one<1, 4>(prm, n_cblk, p->device, stream); break;
+            case 3: st = launch_one<1, 6>(prm, n_cblk, p->device, stream); break;
+            case 4: st = launch_one<1, 8>(prm, n_cblk, p->device, stream); break;
+            case 5: st = launch_one<1, 10>(prm, n_cblk, p->device, stream); break;
+            default: set_error("fused kernel: n_tau %d too large", p->n_tau); return GCAMB_EINVAL;
+        }
+    }
+    if (st != GCAMB_OK) return st;
+    const size_t slice = (size_t)3 * p->n_l * BC;
+    fused_finish_kernel<<<dim3((unsigned)((slice + 255) / 256), (unsigned)n_cblk), 256, 0, stream>>>(
+        scratch, Cl, p->n_bins, p->n_l, n_batch, BC);
+    GCAMB_CUDA(cudaGetLastError());
+    return GCAMB_OK;
+}
+
+}  // namespace gcamb

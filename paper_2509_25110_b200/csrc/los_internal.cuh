@@ -48,6 +48,14 @@ struct gcamb_los_plan {
 
     int32_t order_reversed;  // korder[r] == n_k - 1 - r: a range of positions is a contiguous range of k
 
+    // fused batched path (fused.cu): static, cost-balanced lists of k rows, one per thread block slot
+    int32_t n_bins;          // = n_sm
+    int32_t *d_bin_start;    // [n_bins + 1]
+    int32_t *d_bin_items;    // [n_k] k indices grouped by bin, heaviest first inside a bin
+    // scratch of gcamb_los_spectra_batched (lazily allocated, grow-only)
+    double *d_fused_scratch;
+    size_t fused_scratch_cap;   // bytes
+
     // scratch of gcamb_los_spectra_host (lazily allocated)
     cudaStream_t h_copy, h_comp[4];
     cudaEvent_t h_start, h_copied[4], h_done[4];
@@ -86,6 +94,12 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
 gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
                                    const double *S_E, const double *S_phi, double *Delta,
                                    int pos0, int pos1, bool zero_fill, cudaStream_t stream);
+
+// fused.cu: sources of a batch -> C_l in one kernel (no Delta), for T+E plans whose tau grid fits
+bool fused_supported(const gcamb_los_plan *p, int n_batch);
+size_t fused_scratch_bytes(const gcamb_los_plan *p, int n_batch);
+gcamb_status launch_fused(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
+                          const double *P_R, double *scratch, double *Cl, cudaStream_t stream);
 
 // cls.cu
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,

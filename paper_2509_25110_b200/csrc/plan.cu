@@ -15,6 +15,7 @@
 #include <algorithm>
 #include <cmath>
 #include <numeric>
+#include <queue>
 #include <vector>
 
 #include "los_internal.cuh"
@@ -152,6 +153,35 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     for (int r = 0; r < p->n_k; ++r) p->order_reversed = p->order_reversed && order[r] == p->n_k - 1 - r;
     GCAMB_CUDA(cudaMemcpyAsync(p->d_korder, order.data(), sizeof(int32_t) * p->n_k,
                                cudaMemcpyHostToDevice, stream));
+    // Fused batched path (fused.cu): one static list of k rows per thread-block slot (n_sm of them),
+    // balanced by the longest-processing-time rule on the walked terms plus a per-tile and a per-row
+    // overhead.  Static lists make the order of the k sum of Eq. 1 independent of the scheduling.
+    {
+        p->n_bins = p->n_sm;
+        const long long per_tile = 700, per_row = 20000;   // in walked-term units (ring + flush per tile; prologue)
+        typedef std::pair<long long, int> Load;             // (load, bin): smallest load first
+        std::priority_queue<Load, std::vector<Load>, std::greater<Load>> bins;
+        for (int b = 0; b < p->n_bins; ++b) bins.push(Load(0, b));
+        std::vector<std::vector<int32_t>> items(p->n_bins);
+        for (int r = 0; r < p->n_k; ++r) {
+            const int j = order[r];
+            const long long tiles = std::max(0LL, (long long)p->n_tiles - cost[2 * (size_t)p->n_k + j]);
+            Load top = bins.top();
+            bins.pop();
+            items[top.second].push_back(j);
+            bins.push(Load(top.first + cost[j] + per_tile * tiles + per_row, top.second));
+        }
+        std::vector<int32_t> bin_start(p->n_bins + 1, 0), bin_items;
+        for (int b = 0; b < p->n_bins; ++b) {
+            bin_items.insert(bin_items.end(), items[b].begin(), items[b].end());
+            bin_start[b + 1] = (int32_t)bin_items.size();
+        }
+        GCAMB_CUDA(cudaMalloc(&p->d_bin_start, sizeof(int32_t) * bin_start.size()));
+        GCAMB_CUDA(cudaMalloc(&p->d_bin_items, sizeof(int32_t) * p->n_k));
+        GCAMB_CUDA(cudaMemcpyAsync(p->d_bin_start, bin_start.data(), sizeof(int32_t) * bin_start.size(), cudaMemcpyHostToDevice, stream));
+        GCAMB_CUDA(cudaMemcpyAsync(p->d_bin_items, bin_items.data(), sizeof(int32_t) * p->n_k, cudaMemcpyHostToDevice, stream));
+        GCAMB_CUDA(cudaStreamSynchronize(stream));   // the vectors die with this scope
+    }
     // rows whose largest x = k chi_max exceeds COMP_X_MIN run the compensated coefficient; they
     // must be a prefix of the cost order (they are whenever cost grows with k), else all rows do
     {

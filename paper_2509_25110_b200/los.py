@@ -22,7 +22,7 @@ EXPORTS = (
     "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
-    "gcamb_los_last_error",
+    "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_last_error",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
 PROBE_LIB_PATH = os.path.join(_HERE, "libgcamb_probe.so")
@@ -58,6 +58,9 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_transfer_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_cls_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     lib.gcamb_los_spectra_host.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_spectra_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_spectra_batched_info.argtypes = [_vp, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32),
+                                                   ctypes.POINTER(_i64)]
     _lib = lib
     return lib
 
@@ -166,6 +169,23 @@ class Plan:
         else:
             _check(lib.gcamb_los_cls(self._h, pD, pP, pC, _stream()))
         return out
+
+    def gcamb_los_spectra_batched(self, S_T, S_E, S_phi, P_R, out=None) -> torch.Tensor:
+        """Sources of a batch -> C_l [B][n_spec][n_l] (fused kernel when the plan allows it)."""
+        B = S_T.shape[0]
+        sh = (B, self.n_k, self.n_tau)
+        if out is None:
+            out = torch.empty((B, self.n_spec, self.n_l), dtype=torch.float64, device=S_T.device)
+        _check(load_library().gcamb_los_spectra_batched(
+            self._h, B, _dev(S_T, sh, "S_T"), _dev(S_E, sh, "S_E"), _dev(S_phi, sh, "S_phi"),
+            _dev(P_R, (B, self.n_k), "P_R"), _dev(out, (B, self.n_spec, self.n_l), "Cl"), _stream()))
+        return out
+
+    def gcamb_los_spectra_batched_info(self, n_batch: int) -> dict:
+        fused, kernels, scratch = _i32(), _i32(), _i64()
+        _check(load_library().gcamb_los_spectra_batched_info(self._h, n_batch, ctypes.byref(fused),
+                                                             ctypes.byref(kernels), ctypes.byref(scratch)))
+        return {"fused": bool(fused.value), "kernels": kernels.value, "scratch_bytes": scratch.value}
 
     # ---- host buffers in, host buffers out (H2D + kernels + D2H inside the call)
     def gcamb_los_spectra_host(self, S_T, S_E, S_phi, P_R, Cl_out, Delta_out=None) -> None:
