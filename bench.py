@@ -3,8 +3,11 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
-A step = one pass of the whole hot path, gcamb_los_transfer + gcamb_los_cls (their batched
-forms at config 3), over one batch of seeded synthetic sources that is already resident in HBM.
+A step = one pass of the whole hot path over one batch of seeded synthetic sources that is already
+resident in HBM: gcamb_los_transfer + gcamb_los_cls for a single cosmology; at config 3 (64
+cosmologies, one plan) gcamb_los_spectra_batched, the fused kernel that shares the j_l recurrence
+across the cosmologies of a block and accumulates Eq. 1 without writing Delta (the two-kernel
+batched path is timed beside it).
 Default workload: BASELINE.json config 1 ("CAMB-default-scale", l = 2..2500), the config the
 metric is quoted on.  `value` = nominal (l,k,tau) terms per second = N_l N_k N_tau B per step /
 device time per step (reading R19); the executed-term rate (terms not skipped by R16), spectra/s
@@ -246,19 +249,32 @@ def run_cuda(args) -> None:
     Cl = torch.empty(lead + (plan.n_spec, plan.n_l), dtype=torch.float64, device=dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
 
-    def transfer():
+    fused_info = plan.gcamb_los_spectra_batched_info(B) if batched else {"fused": False}
+    fused = fused_info["fused"]
+
+    def transfer_two_kernel():
         if batched:
             plan.gcamb_los_transfer_batched(dS[0], dS[1], dS[2], out=Delta)
         else:
             plan.gcamb_los_transfer(dS[0], dS[1], dS[2], out=Delta)
 
-    def cls():
+    def cls_two_kernel():
         if batched:
             plan.gcamb_los_cls_batched(Delta, dP, out=Cl)
         else:
             plan.gcamb_los_cls(Delta, dP, out=Cl)
 
-    launches_per_step = plan.launches_per_step
+    if fused:
+        # sources -> C_l in one call (fused kernel + finishing kernel); the "cls" leg is empty
+        def transfer():
+            plan.gcamb_los_spectra_batched(dS[0], dS[1], dS[2], dP, out=Cl)
+
+        def cls():
+            pass
+        launches_per_step = fused_info["kernels"]
+    else:
+        transfer, cls = transfer_two_kernel, cls_two_kernel
+        launches_per_step = plan.launches_per_step
 
     for _ in range(args.warmup):
         flush.zero_()
@@ -283,6 +299,30 @@ def run_cuda(args) -> None:
     t_cls = np.array([e[1].elapsed_time(e[2]) for e in ev]) * 1e-3
     t_step = float(np.mean(t_transfer + t_cls))
 
+    two_kernel = None
+    if fused:   # the same batch through gcamb_los_transfer_batched + gcamb_los_cls_batched, for comparison
+        n2 = max(3, min(args.steps, 10))
+        ev2 = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n2)]
+        transfer_two_kernel()
+        cls_two_kernel()
+        for s in range(n2):
+            flush.zero_()
+            ev2[s][0].record()
+            transfer_two_kernel()
+            ev2[s][1].record()
+            cls_two_kernel()
+            ev2[s][2].record()
+        torch.cuda.synchronize()
+        Cl_two = Cl.clone()
+        transfer()
+        torch.cuda.synchronize()
+        two_kernel = {
+            "transfer_ms": float(np.mean([e[0].elapsed_time(e[1]) for e in ev2])),
+            "cls_ms": float(np.mean([e[1].elapsed_time(e[2]) for e in ev2])),
+            "max_rel_diff_TT_EE": float(((Cl[:, :2] - Cl_two[:, :2]).abs() / Cl_two[:, :2].abs()).max()),
+        }
+        two_kernel["spectra_per_s"] = B / ((two_kernel["transfer_ms"] + two_kernel["cls_ms"]) * 1e-3)
+
     # ---- e2e: the public host-buffer call, H2D of the sources and D2H of C_l inside the timed region
     hCl = torch.empty((B, plan.n_spec, plan.n_l), dtype=torch.float64).pin_memory()
     e2e_steps = max(3, min(args.steps, 20))
@@ -295,7 +335,10 @@ def run_cuda(args) -> None:
     torch.cuda.synchronize()
     t_e2e = (time.perf_counter() - e0) / e2e_steps
     barrier()
-    same = bool(np.array_equal(hCl.numpy().reshape(Cl.shape), Cl.cpu().numpy()))
+    if fused:   # the host entry point runs the two-kernel path: same sums in another order
+        same = bool(np.allclose(hCl.numpy().reshape(Cl.shape), Cl.cpu().numpy(), rtol=1e-9, atol=0.0))
+    else:
+        same = bool(np.array_equal(hCl.numpy().reshape(Cl.shape), Cl.cpu().numpy()))
     h2d = sum(int(x.numel()) * 8 for x in hS if x is not None) + int(hP.numel()) * 8
     d2h = int(hCl.numel()) * 8
 
@@ -305,7 +348,19 @@ def run_cuda(args) -> None:
 
     nominal = plan.nominal_terms * B
     executed = plan.executed_terms * B
-    flop_per_term = 2 * (2 + plan.n_src)             # coefficient + recurrence + n_src accumulate DFMAs
+    if fused:
+        # a block of BC cosmologies shares the coefficient and the recurrence: 2 + n_src BC FP64 lane-slots
+        # per (l, k, tau) for BC cosmologies; executed counts (l, k, tau, cosmology)
+        bc = 8 if (B > 4 and plan.n_tau <= 1280) else 4
+        flop_per_term = 2 * (2 + plan.n_src * bc) / bc
+        kernel_name = "fused_kernel"
+        algorithmic = (f"{flop_per_term} flop per executed (l,k,tau,cosmology): (2 + {plan.n_src} x {bc}) FP64 FMA lane-slots "
+                       f"per (l,k,tau) shared by a block of {bc} cosmologies, x {executed} executed terms per launch; "
+                       f"the time is that of the whole call (fused kernel + finishing kernel)")
+    else:
+        flop_per_term = 2 * (2 + plan.n_src)         # coefficient + recurrence + n_src accumulate DFMAs
+        kernel_name = "transfer_kernel"
+        algorithmic = f"{flop_per_term} flop per executed term x {executed} executed terms per launch"
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     achieved_tf = executed * flop_per_term / t_tr / 1e12
 
@@ -344,18 +399,19 @@ def run_cuda(args) -> None:
         "transfer_ms": 1e3 * t_tr, "cls_ms": 1e3 * t_cl, "plan_create_ms": plan_ms,
         "wall_ms_per_step_incl_flush": 1e3 * wall / args.steps,
         "clocks": clocks,
+        **({"two_kernel_path": two_kernel} if two_kernel else {}),
         "e2e": {"value": nominal * world / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e, "api": "gcamb_los_spectra_host",
                 "matches_device_path": same},
         "gpu_launches": launches_per_step * args.steps,
         "roofline": {
-            "bound": "alu", "kernel": "transfer_kernel", "achieved": achieved_tf, "peak": peak_tf,
+            "bound": "alu", "kernel": kernel_name, "achieved": achieved_tf, "peak": peak_tf,
             "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
             "traffic_unit": "bytes per transfer call (ncu dram read+write, profiles/r1_transfer_kernel_*.txt)",
             "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
                            f"dfma probe measured {probe_tf:.2f} TFLOP/s, dmma (m8n8k4.f64) probe "
                            f"{probe_dmma_tf:.2f} TFLOP/s in this process",
-            "algorithmic": f"{flop_per_term} flop per executed term x {executed} executed terms per launch",
+            "algorithmic": algorithmic,
             "frac_of_measured_dfma": achieved_tf / probe_tf,
         },
     }

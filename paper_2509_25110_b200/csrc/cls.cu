@@ -1,16 +1,17 @@
 // cls.cu -- step a4: C_l^{XY} = 4 pi sum_j dlnk_j P_R(k_j) Delta^X_l(k_j) Delta^Y_l(k_j)
 // (Eq. 1; discrete form BJ, R6, R12).  HBM-bound: Delta is read exactly once,
-// coalesced along k with 16-byte loads.  One CTA takes R consecutive l of one cosmology, so that
-// the weights w_j = dlnk_j P_R(k_j) are formed once per R rows (at one row per CTA the weight reads
-// doubled the L2 -> SM traffic) and every thread has 2 + R n_src independent loads in flight per
-// step.  Fixed-order (deterministic) reduction: thread-private sums over k, shuffle tree, then the
-// warps in index order.
+// coalesced along k with 16-byte loads, four steps of 2 + R n_src independent loads in flight per
+// thread.  One CTA takes R consecutive l of one cosmology (R = 1: see CLS_ROWS below).  Fixed-order
+// (deterministic) reduction: thread-private sums over k, shuffle tree, then the warps in index order.
 #include "los_internal.cuh"
 
 namespace gcamb {
 
-constexpr int CLS_ROWS = 2;               // l rows per CTA (they share the weights)
-constexpr int CLS_THREADS_DEFAULT = 128;
+// Measured on B200 (profiles/README.md, cls section): one row per 256-thread CTA is the fastest shape at
+// every config (rows per CTA 1 / 2 / 4 at config 1: 35 / 39 / 45 us; at config 4: 0.70 / 0.84 / 0.99 ms):
+// more rows per CTA mean fewer, longer-lived CTAs and a coarser tail.
+constexpr int CLS_ROWS = 1;               // l rows per CTA (rows of a CTA share the weights)
+constexpr int CLS_THREADS_DEFAULT = 256;
 
 template <int VEC> struct Pack;
 template <> struct Pack<1> { double v[1]; };
@@ -41,7 +42,7 @@ __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restri
 #pragma unroll
         for (int q = 0; q < NSPEC; ++q) s[r][q] = 0.0;
     const int n_pack = n_k / VEC;
-#pragma unroll 2
+#pragma unroll 4
     for (int j = threadIdx.x; j < n_pack; j += CLS_THREADS) {
         const pack a = dl[j], c = pr[j];
         pack d[R][NSRC];

@@ -176,7 +176,10 @@ __device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T]
     }
 }
 
-template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE>
+// MULTI: the tau range takes several passes (n_tau > threads * T).  A kernel of its own, so that the
+// single-pass kernels carry neither the pass loop nor the load-add-store of the flush (measured:
+// config 1 +4 % with a run-time pass count).
+template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE, bool MULTI>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
     static_assert(T >= 1 && T <= T_MAX, "the NA dispatch below is written out for T <= 12");
@@ -215,8 +218,9 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
 #define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
 
-  for (int pass = 0; pass < p.n_pass; ++pass) {
-    if (pass) {   // the ring and its barriers start afresh; the stores of the previous pass are visible to the whole CTA
+  const int n_pass = MULTI ? p.n_pass : 1;
+  for (int pass = 0; pass < n_pass; ++pass) {
+    if (MULTI && pass) {   // the ring and its barriers start afresh; the stores of the previous pass are visible to the whole CTA
         __syncthreads();
         if (tid == 0)
             for (int d = 0; d < 2 * RD; ++d) { mbar_inval(bar_full + 8 * d); mbar_init(bar_full + 8 * d, W); }
@@ -235,7 +239,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // zero-prefix lengths of the (at most two, normally) Delta rows this CTA zero-fills: looked up here
     // so that the look-ups travel with the prologue loads instead of adding their own round trips
     const int zf_rows = NSRC * p.n_l, zf_step = gridDim.x / p.n_batch;
-    const bool zf = pass == 0 && p.zero_fill;
+    const bool zf = (!MULTI || pass == 0) && p.zero_fill;
     int zf_nz[2] = {0, 0};
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
@@ -344,7 +348,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
                     sum *= f_pref[o];
                     double *dst = p.Delta + DIDX(q, li);
-                    *dst = pass ? *dst + sum : sum;   // pass p adds to what this CTA stored in passes < p
+                    *dst = (MULTI && pass) ? *dst + sum : sum;   // pass p adds to what this CTA stored in passes < p
                 }
             }
             // CTAs smaller than the one NOUT was sized for: the remaining columns
@@ -357,7 +361,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
                     if (q == 1) sum *= p.pref[li];
                     double *dst = p.Delta + DIDX(q, li);
-                    *dst = pass ? *dst + sum : sum;
+                    *dst = (MULTI && pass) ? *dst + sum : sum;
                 }
             }
         }
@@ -468,16 +472,19 @@ constexpr int MINB_256 = 1;
 // Launch shape.  CTA sizes are powers of two of warps (1, 2, 4, 8): the hardware deals
 // a CTA's warps round-robin to the SM's four sub-partitions, each with its own FP64 pipe, and a CTA
 // advances at the pace of its slowest warp, so warp counts such as 5 leave one pipe with twice the
-// work of the others (measured: profiles/README.md).  The tau range is cut into the fewest passes of
-// at most threads * T_MAX points; T is the smallest slot count that covers a pass.
-//   * large launches (enough warps to fill the machine): least padding wins; at equal padding the
-//     smaller CTA, i.e. more points per thread: the cross-thread reduction costs one DADD per thread,
-//     tile row and source whatever T is.  More than 128 threads only when that saves a pass.
-//   * small launches (n_rows CTAs of that shape would leave the SMs' sub-partitions with fewer than
-//     FILL_WARPS warps each): trade points per thread for threads until they do, because a lone warp
-//     per sub-partition runs at the latency of its dependent DFMA chains, not at throughput.
-// The result depends on (n_tau, n_src, n_rows, n_sm) only; the order of every sum depends on the
-// shape, so a batched call and a single call agree bit for bit only when they choose the same shape:
+// work of the others (measured: profiles/README.md).
+//   * n_tau <= 128 T_MAX: one pass; least padding wins, at equal padding the smaller CTA, i.e. more
+//     points per thread (the cross-thread reduction costs one DADD per thread, tile row and source
+//     whatever T is).  Small launches (n_rows CTAs of that shape would leave the SMs' sub-partitions
+//     with fewer than FILL_WARPS warps each) trade points per thread for threads until they do: a
+//     lone warp per sub-partition runs at the latency of its dependent DFMA chains, not at throughput
+//     (config 0: 37 us with one-warp CTAs, 25 us with 128 threads x 3 points).
+//   * n_tau <= 256 T_MAX: one pass of a 256-thread CTA (config 2: 14.8 ms against 15.6 ms for two
+//     passes of 128 threads).
+//   * longer grids: passes of 128 threads x T_MAX points, the last one shorter (config 4: three
+//     passes 52.9 ms, two passes of 256 threads 53.4 ms).
+// The result depends on (n_tau, n_rows, n_sm) only; the order of every sum depends on the shape, so a
+// batched call and a single call agree bit for bit only when they choose the same shape:
 // choose_shape is therefore evaluated with the rows of ONE cosmology (n_k), never with n_k * n_batch.
 #if !defined(GCAMB_TU_SPARSE) || (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
 TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm)
@@ -489,23 +496,20 @@ TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm)
         s.V = TILE_V;
         s.threads = threads;
         s.n_pass = (n_tau + threads * T_MAX - 1) / (threads * T_MAX);
-        s.pass_len = (n_tau + s.n_pass - 1) / s.n_pass;
-        s.T = (s.pass_len + threads - 1) / threads;
+        s.pass_len = s.n_pass > 1 ? threads * T_MAX : n_tau;
+        s.T = s.n_pass > 1 ? T_MAX : (n_tau + threads - 1) / threads;
         return s;
     };
-    auto padding = [&](const TransferShape &s) { return (long long)s.n_pass * s.T * s.threads - n_tau; };
-    TransferShape best = shape_for(32);
-    for (int threads = 64; threads <= 256; threads <<= 1) {
+    auto padding = [&](const TransferShape &s) { return (long long)s.T * s.threads - n_tau; };
+    if (n_tau > 256 * T_MAX) return shape_for(128);
+    if (n_tau > 128 * T_MAX) return shape_for(256);
+    TransferShape best = shape_for(128);
+    for (int threads = 64; threads >= 32; threads >>= 1) {
         const TransferShape s = shape_for(threads);
-        if (threads == 256 && s.n_pass >= best.n_pass) break;
-        if (s.n_pass < best.n_pass || (s.n_pass == best.n_pass && padding(s) < padding(best))) best = s;
+        if (s.n_pass == 1 && padding(s) <= padding(best)) best = s;
     }
     const long long want = (long long)FILL_WARPS * 4 * n_sm;
-    while (best.threads < 256 && best.T >= 4 && n_rows * (best.threads / 32) < want) {
-        const TransferShape s = shape_for(best.threads * 2);
-        if (s.n_pass > best.n_pass) break;
-        best = s;
-    }
+    while (best.threads < 256 && best.T >= 4 && n_rows * (best.threads / 32) < want) best = shape_for(best.threads * 2);
     return best;
 }
 #endif
@@ -530,15 +534,22 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     // are compiled for 3 co-resident CTAs per SM (168 registers) while that fits, else for 2
     constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : MINB_128;
     const bool small = sh.threads <= 128;
-    auto kern = small ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE>
-                      : transfer_kernel<T, V, NSRC, RING_G, 256, MINB_256, COMP, SPARSE>;
+    // multi-pass launches always run 128 threads x T_MAX points (choose_shape): one more kernel, not 24
+    const bool multi = sh.n_pass > 1;
+    if (multi && !(T == T_MAX && small)) { set_error("internal: multi-pass shape %d x %d", sh.threads, T); return GCAMB_EINVAL; }
+    void (*kern)(TransferParams) = small ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, false>
+                                         : transfer_kernel<T, V, NSRC, RING_G, 256, MINB_256, COMP, SPARSE, false>;
+    if constexpr (T == T_MAX) {
+        if (multi) kern = transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, true>;
+    }
     // opt in to large dynamic shared memory once per kernel and device (bit d of the mask = device d done)
-    static std::atomic<unsigned long long> attr_done[2];
+    static std::atomic<unsigned long long> attr_done[3];
+    const int which = multi ? 2 : small;
     const unsigned long long dev_bit = 1ull << (device & 63);
-    if (!(attr_done[small].load(std::memory_order_acquire) & dev_bit)) {
+    if (!(attr_done[which].load(std::memory_order_acquire) & dev_bit)) {
         GCAMB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)smem_bytes(small ? 128 : 256)));
-        attr_done[small].fetch_or(dev_bit, std::memory_order_release);
+        attr_done[which].fetch_or(dev_bit, std::memory_order_release);
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(n_pos * prm.n_batch));

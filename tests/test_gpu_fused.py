@@ -93,13 +93,29 @@ def test_fused_does_not_depend_on_the_other_cosmologies(los):
     plan.close()
 
 
-@pytest.mark.parametrize("case", ["phi", "sparse_l", "single", "long_tau"])
+def test_fused_with_a_sparse_l_list(los):
+    """CAMB's default operating mode (`l_sample_boost`): only the listed l are accumulated."""
+    cfg = synth.Config(9, "fused-sparse", 2, 700, 30, 1e-4, 0.3, 150, 80, False, n_batch=6)
+    l_list = np.unique(np.concatenate([np.arange(2, 20), np.arange(20, 100, 10), np.arange(100, 701, 50)])).astype(np.int32)
+    hS, hP = batch_inputs(cfg)
+    plan = los.Plan(l_list, cfg.k(), cfg.tau(), cfg.tau0)
+    assert plan.gcamb_los_spectra_batched_info(6)["fused"]
+    C = plan.gcamb_los_spectra_batched(dev(hS[0]), dev(hS[1]), None, dev(hP)).cpu().numpy()
+    for c in (0, 5):
+        D_ref = oracle.transfer(l_list, cfg.k(), cfg.tau(), cfg.tau0, hS[0][c], hS[1][c], real="f80")
+        C_ref = oracle.cls(cfg.k(), D_ref, hP[c], real="f80")
+        e_auto, e_te = cl_err(C[c], C_ref)
+        assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
+@pytest.mark.parametrize("case", ["phi", "single", "long_tau"])
 def test_plans_outside_the_fused_kernel_take_the_two_kernel_path(los, case):
     with_phi = case == "phi"
     B = 1 if case == "single" else 4
     n_u, n_log = (1500, 1200) if case == "long_tau" else (100, 60)
     cfg = synth.Config(9, "fallback", 2, 120, 20, 1e-4, 0.2, n_u, n_log, with_phi, n_batch=B)
-    l_list = cfg.l_list()[::7].copy() if case == "sparse_l" else cfg.l_list()
+    l_list = cfg.l_list()
     hS, hP = batch_inputs(cfg)
     plan = los.Plan(l_list, cfg.k(), cfg.tau(), cfg.tau0, with_phi=with_phi)
     info = plan.gcamb_los_spectra_batched_info(B)
