@@ -136,6 +136,23 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
                                    void *cuda_stream);
 
 /*
+ * Spectra on EVERY multipole l_list[0] .. l_list[n_l-1] from the spectra on the plan's (sparse) l list:
+ * CAMB computes "a number of explicitly computed multipoles" set by l_sample_boost and obtains the
+ * others by "spline interpolation" (footnote 5 PAPER.md:127).  The paper
+ * defines neither the spline nor the interpolated quantity; reading R25: NATURAL cubic
+ * spline in l (second derivative 0 at both ends) of y(l) = l (l+1) C_l^{XY}, knots = the l list,
+ * every spectrum alike, C_l = y(l) / (l (l+1)) afterwards.  The listed multipoles come back
+ * unchanged up to rounding (y_i / (l_i (l_i+1))).  The LU factors of the spline's tridiagonal system
+ * depend on the l list only and are plan tables; a call runs one kernel, one thread block per
+ * (cosmology, spectrum).  Needs 2 <= n_l <= 12800 (GCAMB_EINVAL otherwise).
+ *   d_Cl     DEVICE [n_batch][n_spec][n_l]                     as written by gcamb_los_cls[_batched]
+ *   d_Cl_all DEVICE [n_batch][n_spec][l_list[n_l-1] - l_list[0] + 1], one entry per integer l
+ * Asynchronous on `cuda_stream`; deterministic.
+ */
+gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Cl,
+                                 double *d_Cl_all, void *cuda_stream);
+
+/*
  * Batched sources -> spectra in one call, WITHOUT the transfer functions ever reaching memory
  * (the emulator-training use-case: 1e5-1e6 spectra on a fixed grid; Eq. 1-3,
  * PAPER.md:50-58).  For plans with the T and E sources only and n_tau <= 2560 this runs ONE fused

@@ -53,6 +53,7 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile); cudaFree(p->d_inv);
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
+    cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     if (p->h_streams_ready) {
@@ -180,6 +181,7 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (e != cudaSuccess) { gcamb_status st = cuda_fail(e, "plan tables"); free_plan(p); return st; }
 
     gcamb_status st = plan_precompute(p, stream);
+    if (st == GCAMB_OK) st = interp_plan_tables(p, l_list, stream);
     if (st != GCAMB_OK) { free_plan(p); return st; }
     *out = p;
     return GCAMB_OK;
@@ -249,6 +251,15 @@ gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, co
                            double *d_Cl, void *cuda_stream)
 {
     return gcamb_los_cls_batched(plan, 1, d_Delta, d_P_R, d_Cl, cuda_stream);
+}
+
+gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Cl,
+                                 double *d_Cl_all, void *cuda_stream)
+{
+    if (!plan || !d_Cl || !d_Cl_all) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(plan)) return st;
+    return launch_cl_interp(plan, n_batch, d_Cl, d_Cl_all, (cudaStream_t)cuda_stream);
 }
 
 gcamb_status gcamb_los_spectra_batched(gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,

@@ -56,6 +56,11 @@ struct gcamb_los_plan {
     double *d_fused_scratch;
     size_t fused_scratch_cap;   // bytes
 
+    // interpolation in l (interp.cu, reading R25): LU factors of the natural-spline system of the l list
+    double *d_sp_mult;       // [n_l] forward-elimination multipliers
+    double *d_sp_inv_diag;   // [n_l] reciprocals of the eliminated diagonal
+    int32_t *d_sp_seg;       // [l_max - l_min + 1] knot interval of every integer l
+
     // scratch of gcamb_los_spectra_host (lazily allocated)
     cudaStream_t h_copy, h_comp[4];
     cudaEvent_t h_start, h_copied[4], h_done[4];
@@ -100,6 +105,12 @@ bool fused_supported(const gcamb_los_plan *p, int n_batch);
 size_t fused_scratch_bytes(const gcamb_los_plan *p, int n_batch);
 gcamb_status launch_fused(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
                           const double *P_R, double *scratch, double *Cl, cudaStream_t stream);
+
+// interp.cu: C_l on every integer l of [l_min, l_max] from C_l on the l list (natural cubic spline of l(l+1) C_l)
+constexpr size_t INTERP_SMEM_MAX = 200 * 1024;   // two doubles per knot in shared memory: n_l <= 12800
+gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaStream_t stream);
+gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double *Cl_samp, double *Cl_all,
+                              cudaStream_t stream);
 
 // cls.cu
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,

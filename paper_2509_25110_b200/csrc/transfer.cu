@@ -142,7 +142,8 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
             const double tl = tl0 - 2.0 * s;   // 2l+1
             const double c = COMP ? fma(tl, ix[j], e) : tl * ix[j];
 #pragma unroll
-            for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
+            for (int q = 0; q < NSRC; ++q)   // the first slot starts the sums: no zeroing of the accumulators
+                acc[q][s] = j == 0 ? src[q][j] * fb[j] : fma(src[q][j], fb[j], acc[q][s]);
             const double fn = fma(c, fb[j], -fa[j]);
             fa[j] = fb[j];
             fb[j] = fn;
@@ -185,20 +186,23 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     static_assert(T >= 1 && T <= T_MAX, "the NA dispatch below is written out for T <= 12");
     constexpr int P = NSRC * V;          // partial sums per thread and tile
     constexpr int NOUT = (G * P + MAXTHREADS - 1) / MAXTHREADS;   // flush outputs per thread (full CTA)
-    // start pairs [T][threads] | transpose scratch [W][32][P+2] | ring [2][G][W][P] |
-    // start tiles [T][threads] | slot first/last start tile [W][2T]
+    // Shared memory, laid out with the compile-time strides of a full CTA (NT threads, WM warps) whatever
+    // blockDim is, so that every address is a constant offset from a per-thread base:
+    // start pairs [T][NT] | transpose scratch [WM][32][P+2] | ring [RD][G][WM][P] | barriers [2 RD] |
+    // start tiles [T][NT] | slot first/last start tile [WM][2T] | (COMP) reciprocal residuals [T][NT]
+    constexpr int NT = MAXTHREADS, WM = NT / 32;
     extern __shared__ double2 smem2[];
     const int tid = threadIdx.x, lane = tid & 31, W = blockDim.x >> 5;
     const int warp = __reduce_min_sync(0xffffffffu, tid >> 5);   // through a warp reduction: uniform register
-    double2 *my_start = smem2 + tid;     // [j * blockDim]: private to this thread, no barrier needed
-    double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)warp * 32 * (P + 2);
-    double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * blockDim.x) + (size_t)W * 32 * (P + 2);
-    int *my_tile = reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) + tid;   // [j * blockDim]
-    int *slot_win = reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) + (size_t)T * blockDim.x + warp * 2 * T;
-    // compensated rows only: residuals of the rounded reciprocals [T][threads], after the (8-byte aligned) int tables
-    double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)RD * G * W * P + 2 * RD) +
-                                                 (((size_t)T * blockDim.x + W * 2 * T + 1) & ~(size_t)1)) + tid;
-    const uint32_t bar_full = (uint32_t)__cvta_generic_to_shared(ring + (size_t)RD * G * W * P);
+    double2 *my_start = smem2 + tid;     // [j * NT]: private to this thread, no barrier needed
+    double *scratch = reinterpret_cast<double *>(smem2 + (size_t)T * NT) + (size_t)warp * 32 * (P + 2);
+    double *ring = reinterpret_cast<double *>(smem2 + (size_t)T * NT) + (size_t)WM * 32 * (P + 2);
+    int *my_tile = reinterpret_cast<int *>(ring + (size_t)RD * G * WM * P + 2 * RD) + tid;   // [j * NT]
+    int *slot_win = reinterpret_cast<int *>(ring + (size_t)RD * G * WM * P + 2 * RD) + (size_t)T * NT + warp * 2 * T;
+    // compensated rows only: residuals of the rounded reciprocals [T][NT], after the (8-byte aligned) int tables
+    double *my_ixlo = reinterpret_cast<double *>(reinterpret_cast<int *>(ring + (size_t)RD * G * WM * P + 2 * RD) +
+                                                 (((size_t)T * NT + WM * 2 * T + 1) & ~(size_t)1)) + tid;
+    const uint32_t bar_full = (uint32_t)__cvta_generic_to_shared(ring + (size_t)RD * G * WM * P);
     const uint32_t bar_empty = bar_full + 8 * RD;
     if (tid == 0) for (int d = 0; d < 2 * RD; ++d) mbar_init(bar_full + 8 * d, W);
     __syncthreads();
@@ -270,14 +274,14 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         if (comp) {   // 1/x = inv + inv_lo,  inv_lo = -inv * (inv x - 1), the residual taken exactly by the fma
             const double x = __dmul_rn(kval, p.chi[ic]);
             const double res = fma(inv, x, -1.0);
-            my_ixlo[j * blockDim.x] = valid ? -inv * res : 0.0;
+            my_ixlo[j * NT] = valid ? -inv * res : 0.0;
         }
         tp[j] = valid ? p.tile[row + ic] : NEVER;
-        my_start[j * blockDim.x] = p.start[row + ic];   // never injected when the slot is masked (tile NEVER)
+        my_start[j * NT] = p.start[row + ic];   // never injected when the slot is masked (tile NEVER)
         src[0][j] = w * p.S[0][sx];
         src[1][j] = w * p.S[1][sx] * (inv * inv);
         if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
-        my_tile[j * blockDim.x] = tp[j];
+        my_tile[j * NT] = tp[j];
     }
 #pragma unroll
     for (int j = 0; j < T; ++j) {
@@ -337,7 +341,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         if (has) {
             flush_columns(t_first);
             mbar_wait(bar_full + 8 * stage, (m / RD) & 1);
-            const double *fbuf = ring + (size_t)stage * G * W * P;
+            const double *fbuf = ring + (size_t)stage * G * WM * P;
 #pragma unroll
             for (int o = 0; o < NOUT; ++o) {
                 const int idx = tid + o * (int)blockDim.x;
@@ -345,7 +349,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                 if (idx < gcount * P && li >= 0) {
                     const int gi = idx / P, r = idx - gi * P, q = r / V;
                     double sum = 0.0;
-                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * WM + wv) * P + r];
                     sum *= f_pref[o];
                     double *dst = p.Delta + DIDX(q, li);
                     *dst = (MULTI && pass) ? *dst + sum : sum;   // pass p adds to what this CTA stored in passes < p
@@ -358,7 +362,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                 const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
                 if (li >= 0) {
                     double sum = 0.0;
-                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * W + wv) * P + r];
+                    for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * WM + wv) * P + r];
                     if (q == 1) sum *= p.pref[li];
                     double *dst = p.Delta + DIDX(q, li);
                     *dst = (MULTI && pass) ? *dst + sum : sum;
@@ -398,8 +402,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         if (inj_from <= t) {
 #pragma unroll
             for (int j = 0; j < T; ++j) {
-                if (my_tile[j * blockDim.x] == t) {
-                    const double2 st = my_start[j * blockDim.x];
+                if (my_tile[j * NT] == t) {
+                    const double2 st = my_start[j * NT];
                     fa[j] = st.x;
                     fb[j] = st.y;
                 }
@@ -414,22 +418,18 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             acc_on = (mask_word >> (t & 31)) & 1u;
             g_any |= acc_on;
         }
-        double *rb = ring + ((size_t)((n % RD) * G + g) * W + warp) * P;   // summed by warp index: a fixed order
+        double *rb = ring + ((size_t)((n % RD) * G + g) * WM + warp) * P;   // summed by warp index: a fixed order
         GCAMB_ASSERT(g >= 0 && g < G && warp < W && t >= 0 && na <= T && n * G + g == t - t_begin);
         if (SPARSE && !acc_on) {
-#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C>(tl0, ix, my_ixlo, blockDim.x, fa, fb); break;
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C>(tl0, ix, my_ixlo, NT, fa, fb); break;
             switch (na) {
                 GCAMB_NA(1, COMP) GCAMB_NA(2, COMP) GCAMB_NA(3, COMP) GCAMB_NA(4, COMP) GCAMB_NA(5, COMP) GCAMB_NA(6, COMP)
                 GCAMB_NA(7, COMP) GCAMB_NA(8, COMP) GCAMB_NA(9, COMP) GCAMB_NA(10, COMP) GCAMB_NA(11, COMP) GCAMB_NA(12, COMP)
             }
 #undef GCAMB_NA
         } else if (na > 0) {
-            double acc[NSRC][V];
-#pragma unroll
-            for (int q = 0; q < NSRC; ++q)
-#pragma unroll
-                for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
-#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, blockDim.x, src, fa, fb, acc); break;
+            double acc[NSRC][V];   // written by the first slot of the tile body
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, NT, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
                 GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) \
@@ -522,6 +522,7 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     if (n_pos <= 0) return GCAMB_OK;
     prm.k_first = k_first;
     prm.zero_fill = zero_fill;
+    // shared memory of a full CTA (the layout uses the compile-time strides whatever the launch size)
     auto smem_bytes = [](int threads) {
         const int W = threads / 32;
         size_t smem = sizeof(double2) * T * threads + sizeof(double) * W * 32 * (NSRC * V + 2) +
@@ -554,7 +555,7 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(n_pos * prm.n_batch));
     cfg.blockDim = dim3((unsigned)sh.threads);
-    cfg.dynamicSmemBytes = smem_bytes(sh.threads);
+    cfg.dynamicSmemBytes = smem_bytes(small ? 128 : 256);
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

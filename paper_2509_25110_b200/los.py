@@ -22,7 +22,7 @@ EXPORTS = (
     "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
-    "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_last_error",
+    "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
 PROBE_LIB_PATH = os.path.join(_HERE, "libgcamb_probe.so")
@@ -61,6 +61,7 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_spectra_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_spectra_batched_info.argtypes = [_vp, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32),
                                                    ctypes.POINTER(_i64)]
+    lib.gcamb_los_cl_interp.argtypes = [_vp, _i32, _vp, _vp, _vp]
     _lib = lib
     return lib
 
@@ -116,6 +117,7 @@ class Plan:
         ex = _i64()
         _check(lib.gcamb_los_plan_info(self._h, *[ctypes.byref(o) for o in out], ctypes.byref(ex)))
         self.n_l, self.n_k, self.n_tau, self.n_src, self.n_spec = (o.value for o in out)
+        self.n_l_all = int(l_list[-1] - l_list[0] + 1)      # integer multipoles spanned by the l list
         self.executed_terms = ex.value
         self.nominal_terms = self.n_l * self.n_k * self.n_tau
         # kernels of this library one transfer + one cls call launch (bench.py's gpu_launches)
@@ -168,6 +170,17 @@ class Plan:
             _check(lib.gcamb_los_cls_batched(self._h, B[0], pD, pP, pC, _stream()))
         else:
             _check(lib.gcamb_los_cls(self._h, pD, pP, pC, _stream()))
+        return out
+
+    def gcamb_los_cl_interp(self, Cl, out=None) -> torch.Tensor:
+        """C_l on the l list [..., n_spec, n_l] -> C_l on every integer l [..., n_spec, l_last - l_first + 1]."""
+        lead = tuple(Cl.shape[:-2])
+        n_batch = int(np.prod(lead)) if lead else 1
+        if out is None:
+            out = torch.empty(lead + (self.n_spec, self.n_l_all), dtype=torch.float64, device=Cl.device)
+        _check(load_library().gcamb_los_cl_interp(
+            self._h, n_batch, _dev(Cl, lead + (self.n_spec, self.n_l), "Cl"),
+            _dev(out, lead + (self.n_spec, self.n_l_all), "Cl_all"), _stream()))
         return out
 
     def gcamb_los_spectra_batched(self, S_T, S_E, S_phi, P_R, out=None) -> torch.Tensor:

@@ -226,6 +226,42 @@ def test_single_tau_source_is_the_kernel(los):
         assert np.max(np.abs(D[0, :, j] - jl)) <= 3e-12 / max(x, 1.0) + 1e-300
         assert np.array_equal(D[2, :, j], D[0, :, j])
 
+# --------------------------------------------------------------------------- C_l kernels alone (a4)
+@pytest.mark.parametrize("shape", [
+    # (n_k, n_l, batch, with_phi): the streaming kernel (n_k even, <= 6144) at its chunk boundaries,
+    # with more rows than SMs, fewer rows than SMs, CTA row ranges that straddle cosmologies;
+    # the row-per-CTA kernel for odd and long rows
+    (1536, 40, 1, False), (1538, 7, 3, True), (3000, 300, 1, False), (3072, 33, 5, False),
+    (6144, 12, 2, True), (2, 9, 4, False), (50, 700, 3, True),
+    (6146, 10, 2, False), (1537, 21, 2, True), (20000, 6, 1, True),
+])
+def test_cls_kernels_on_random_transfer_functions(los, shape):
+    """Eq. 1 alone, on random Delta (no structure a wrong index could hide behind): element by element
+    against the long-double oracle, batched == loop of single calls bit for bit, run-to-run bit equality."""
+    n_k, n_l, B, with_phi = shape
+    rng = np.random.default_rng(n_k + n_l)
+    k = np.geomspace(1e-4, 0.5, n_k) * (1.0 + 0.1 * rng.uniform(size=n_k) / n_k)     # non-uniform ln k steps
+    k = np.sort(k)
+    tau = np.array([100.0, 5000.0, 13000.0])
+    l_list = np.arange(2, 2 + n_l, dtype=np.int32)
+    plan = los.Plan(l_list, k, tau, 14000.0, with_phi=with_phi)
+    D = rng.standard_normal((B, plan.n_src, n_l, n_k))
+    P = rng.uniform(1e-9, 3e-9, size=(B, n_k))
+    d_D, d_P = dev(D), dev(P)
+    C = torch.full((B, plan.n_spec, n_l), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_cls_batched(d_D, d_P, out=C)
+    torch.cuda.synchronize()
+    C_h = C.cpu().numpy()
+    for b in range(B):
+        C_ref = oracle.cls(k, D[b], P[b], real="f80")
+        auto = [0, 1] + ([3] if with_phi else [])
+        assert np.max(np.abs(C_h[b][auto] / C_ref[auto] - 1.0)) <= 1e-13
+        norm = np.sqrt(C_ref[0] * C_ref[1])
+        assert np.max(np.abs(C_h[b][2] - C_ref[2]) / norm) <= 1e-13
+        assert torch.equal(plan.gcamb_los_cls(d_D[b], d_P[b]), C[b])
+    assert torch.equal(plan.gcamb_los_cls_batched(d_D, d_P), C)
+    plan.close()
+
 
 # --------------------------------------------------------------------------- batched == loop of single
 def test_batched_equals_loop_of_single(los):
