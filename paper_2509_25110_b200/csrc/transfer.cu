@@ -142,8 +142,7 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
             const double tl = tl0 - 2.0 * s;   // 2l+1
             const double c = COMP ? fma(tl, ix[j], e) : tl * ix[j];
 #pragma unroll
-            for (int q = 0; q < NSRC; ++q)   // the first slot starts the sums: no zeroing of the accumulators
-                acc[q][s] = j == 0 ? src[q][j] * fb[j] : fma(src[q][j], fb[j], acc[q][s]);
+            for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
             const double fn = fma(c, fb[j], -fa[j]);
             fa[j] = fb[j];
             fb[j] = fn;
@@ -428,7 +427,11 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             }
 #undef GCAMB_NA
         } else if (na > 0) {
-            double acc[NSRC][V];   // written by the first slot of the tile body
+            double acc[NSRC][V];
+#pragma unroll
+            for (int q = 0; q < NSRC; ++q)
+#pragma unroll
+                for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
 #define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, NT, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
