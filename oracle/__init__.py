@@ -56,6 +56,11 @@ def _lib(real: str) -> ctypes.CDLL:
             lib.oracle_cls.argtypes = [ctypes.c_int, ctypes.c_int, _pd, ctypes.c_int, _pd, _pd,
                                        ctypes.c_int, _pd]
             lib.oracle_cl_interp.argtypes = [_pi, ctypes.c_int, ctypes.c_int, _pd, _pd]
+            lib.oracle_sph_bessel_derivs.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_transfer_tensor.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
+                                                   ctypes.c_double, _pd, _pd, _pd, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_cls_tensor.argtypes = [ctypes.c_int, _pd, ctypes.c_int, _pd, _pd, ctypes.c_int, _pd]
+            lib.oracle_interp_sources.argtypes = [_pd, ctypes.c_int, _pd, ctypes.c_int, ctypes.c_int, _pd, _pd]
             assert lib.oracle_real_mant_bits() == (53 if real == "f64" else 64)
             _LIBS[real] = lib
         return _LIBS[real]
@@ -136,4 +141,52 @@ def cl_interp(l_list, Cl_samp, real: str = "f64") -> np.ndarray:
     rc = _lib(real).oracle_cl_interp(l_list.ctypes.data_as(_pi), n_l, n_spec, _ptr(Cl_samp), _ptr(out))
     if rc:
         raise ValueError(f"oracle_cl_interp failed ({rc})")
+    return out
+
+
+def sph_bessel_derivs(x: float, lmax: int, margin: int = DEFAULT_MARGIN, real: str = "f64") -> np.ndarray:
+    """[3][lmax+1]: j_l(x), j_l'(x), j_l''(x), l = 0..lmax (the derivatives are those the tensor kernels use)."""
+    out = np.empty((3, lmax + 1), dtype=np.float64)
+    if _lib(real).oracle_sph_bessel_derivs(float(x), int(lmax), int(margin), _ptr(out)):
+        raise ValueError("oracle_sph_bessel_derivs: bad arguments")
+    return out
+
+
+def transfer_tensor(l_list, k, tau, tau0, S_T, S_E, S_B, margin: int = DEFAULT_MARGIN,
+                    real: str = "f64", nthreads: int = 0) -> np.ndarray:
+    """Tensor transfer functions Delta[3][n_l][n_k], order T, E, B (reading R27)."""
+    l_list = np.ascontiguousarray(l_list, dtype=np.int32)
+    k, tau, S_T, S_E, S_B = _f64(k), _f64(tau), _f64(S_T), _f64(S_E), _f64(S_B)
+    assert S_T.shape == (k.size, tau.size) and S_E.shape == S_T.shape and S_B.shape == S_T.shape
+    out = np.empty((3, l_list.size, k.size), dtype=np.float64)
+    rc = _lib(real).oracle_transfer_tensor(l_list.ctypes.data_as(_pi), l_list.size, _ptr(k), k.size,
+                                           _ptr(tau), tau.size, float(tau0), _ptr(S_T), _ptr(S_E), _ptr(S_B),
+                                           int(margin), int(nthreads), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_transfer_tensor failed ({rc})")
+    return out
+
+
+def cls_tensor(k, Delta, P_t, real: str = "f64", nthreads: int = 0) -> np.ndarray:
+    """Tensor spectra C_l[4][n_l], order TT, EE, BB, TE (Eq. 1 with P_t, reading R27)."""
+    k, Delta, P_t = _f64(k), _f64(Delta), _f64(P_t)
+    n_src, n_l, n_k = Delta.shape
+    assert n_src == 3 and n_k == k.size == P_t.size
+    out = np.empty((4, n_l), dtype=np.float64)
+    rc = _lib(real).oracle_cls_tensor(n_l, _ptr(k), n_k, _ptr(Delta), _ptr(P_t), int(nthreads), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_cls_tensor failed ({rc})")
+    return out
+
+
+def interp_sources(k_coarse, k, S_coarse, real: str = "f64") -> np.ndarray:
+    """Sources on a coarse k grid [n_kc][n_tau] -> sources on k [n_k][n_tau]: natural cubic spline in k for
+    every tau (reading R26)."""
+    k_coarse, k, S_coarse = _f64(k_coarse), _f64(k), _f64(S_coarse)
+    n_kc, n_tau = S_coarse.shape
+    assert n_kc == k_coarse.size
+    out = np.empty((k.size, n_tau), dtype=np.float64)
+    rc = _lib(real).oracle_interp_sources(_ptr(k_coarse), n_kc, _ptr(k), k.size, n_tau, _ptr(S_coarse), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_interp_sources failed ({rc})")
     return out
