@@ -46,8 +46,9 @@ typedef enum {
     GCAMB_ECUDA = 4   /* any other CUDA error (message in gcamb_los_last_error) */
 } gcamb_status;
 
-/* source mask bits; T and E are mandatory, phi optional (BJ: "TT/EE/TE/phiphi") */
-enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4 };
+/* source mask bits; T and E are mandatory, phi optional (BJ: "TT/EE/TE/phiphi").  GCAMB_SRC_TENSOR alone
+ * makes a tensor-mode plan (sources T, E, B of the tensor perturbations; see gcamb_los_transfer_tensor). */
+enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4, GCAMB_SRC_TENSOR = 8 };
 
 /*
  * Plan creation = `IntegrationVars_init` hoisted out of the per-call path:
@@ -65,7 +66,9 @@ enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4 };
  *   k       HOST [n_k]   strictly increasing, > 0, finite; n_k >= 2 (and n_k * n_batch < 2^31 in
  *                        the batched calls: one thread block per k row and cosmology)
  *   tau     HOST [n_tau] strictly increasing, < tau0, finite; n_tau >= 2
- *   src_mask             GCAMB_SRC_T|GCAMB_SRC_E or GCAMB_SRC_T|GCAMB_SRC_E|GCAMB_SRC_PHI
+ *   src_mask             GCAMB_SRC_T|GCAMB_SRC_E, GCAMB_SRC_T|GCAMB_SRC_E|GCAMB_SRC_PHI, or GCAMB_SRC_TENSOR
+ *                        (tensor plan: l <= 65534, three sources, four spectra; only the *_tensor calls,
+ *                        gcamb_los_cl_interp and gcamb_los_srcinterp_create accept it)
  *   cuda_stream          stream the precompute kernels run on; the call synchronises it.
  * On success *out owns device memory on the CURRENT device; free with gcamb_los_plan_destroy.
  * Every later call on the plan must be made with that device current (GCAMB_EINVAL otherwise;
@@ -151,6 +154,55 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
  */
 gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Cl,
                                  double *d_Cl_all, void *cuda_stream);
+
+/*
+ * Tensor modes: the paper runs SourceToTransfers twice, "one for scalar perturbations
+ * and the other for tensor ones" (Figure 1; get_tensor_cls, l_max_tensor = 1500,
+ * PAPER.md:91-93) and says that for tensors and B modes "similar equations arise" (citing
+ * Seljak & Zaldarriaga) without printing them.  Reading R27: the flat-space
+ * tensor line-of-sight kernels of that literature (Zaldarriaga & Seljak 1997, Eq. 30), x = k (tau0 - tau):
+ *   Delta^{T,t}_l(k) = sqrt((l+2)!/(l-2)!) sum_i w_i S_T(k,tau_i) j_l(x_i) / x_i^2
+ *   Delta^{E,t}_l(k) = sum_i w_i S_E(k,tau_i) [ -j_l + j_l'' + 2 j_l/x^2 + 4 j_l'/x ](x_i)
+ *   Delta^{B,t}_l(k) = sum_i w_i S_B(k,tau_i) [ 2 j_l' + 4 j_l/x ](x_i)
+ *   C_l^{XY,t}       = 4 pi sum_j dlnk_j P_t(k_j) Delta^{X,t}_l(k_j) Delta^{Y,t}_l(k_j),  XY = TT, EE, BB, TE
+ * (Eq. 1 with the tensor primordial spectrum; convention constants of the tensor normalisation belong to
+ * P_t).  `plan` must have been created with src_mask = GCAMB_SRC_TENSOR.  The transfer call runs the
+ * three-source transfer kernels twice on the union of {l} and {l + 1} (the E and B kernels are
+ * combinations of plain j_l and j_{l+1} sums with l-dependent coefficients) plus two small kernels; it
+ * needs caller-owned scratch of gcamb_los_tensor_work_bytes() bytes.  Single cosmology.
+ *   d_S_T, d_S_E, d_S_B DEVICE [n_k][n_tau];  d_Delta DEVICE [3][n_l][n_k], order T, E, B;
+ *   d_work DEVICE scratch;  d_P_t DEVICE [n_k];  d_Cl DEVICE [4][n_l], order TT, EE, BB, TE.
+ * Asynchronous on `cuda_stream`; deterministic.
+ */
+gcamb_status gcamb_los_tensor_work_bytes(const gcamb_los_plan *plan, int64_t *bytes);
+gcamb_status gcamb_los_transfer_tensor(const gcamb_los_plan *plan, const double *d_S_T, const double *d_S_E,
+                                       const double *d_S_B, double *d_Delta, double *d_work,
+                                       void *cuda_stream);
+gcamb_status gcamb_los_cls_tensor(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_t,
+                                  double *d_Cl, void *cuda_stream);
+
+/*
+ * InterpolateSources (SourceToTransfers "begins by calling IntegrationVars_init ... and
+ * InterpolateSources to prepare the source data"): sources known on a coarse wavenumber grid (the modes the
+ * perturbation evolution integrated) -> sources on the plan's k grid.  The paper does not define the
+ * interpolation; reading R26: for every tau independently, the NATURAL cubic spline in k
+ * through the coarse samples.  The handle holds the LU factors of the spline system and, per fine k, its
+ * coarse interval and weights (tables built on the host at creation); it refers to the plan's grids only
+ * at creation and may outlive the plan.
+ *   k_coarse   HOST [n_kc] strictly increasing, > 0; every k of the plan must lie inside
+ *              [k_coarse[0], k_coarse[n_kc-1]] (GCAMB_EGRID otherwise: no extrapolation); n_kc >= 2
+ *   n_series   number of independent [n_kc][n_tau] arrays (sources x cosmologies), <= 65535
+ *   d_S_coarse DEVICE [n_series][n_kc][n_tau];  d_S_fine DEVICE [n_series][n_k][n_tau] (n_k <= 65535)
+ *   d_work     DEVICE scratch of the size of d_S_coarse (second derivatives of the splines)
+ * Asynchronous on `cuda_stream`; two kernels; deterministic.
+ */
+typedef struct gcamb_los_srcinterp gcamb_los_srcinterp;
+gcamb_status gcamb_los_srcinterp_create(gcamb_los_srcinterp **out, const gcamb_los_plan *plan,
+                                        const double *k_coarse, int32_t n_kc, void *cuda_stream);
+gcamb_status gcamb_los_srcinterp_destroy(gcamb_los_srcinterp *handle);
+gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *handle, int32_t n_series,
+                                      const double *d_S_coarse, double *d_S_fine, double *d_work,
+                                      void *cuda_stream);
 
 /*
  * Batched sources -> spectra in one call, WITHOUT the transfer functions ever reaching memory

@@ -18,7 +18,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgcamb_los.so")
 PROBE_LIB = os.path.join(HERE, "libgcamb_probe.so")
 # (source, extra flags, object tag): transfer.cu is compiled once per (sparse, n_src) entry, in parallel
-UNITS = [("api.cu", [], "api"), ("plan.cu", [], "plan"), ("cls.cu", [], "cls"), ("fused.cu", [], "fused"), ("interp.cu", [], "interp")] + [
+UNITS = [("api.cu", [], "api"), ("plan.cu", [], "plan"), ("cls.cu", [], "cls"), ("fused.cu", [], "fused"), ("interp.cu", [], "interp"), ("tensor.cu", [], "tensor"),
+         ("srcinterp.cu", [], "srcinterp")] + [
     ("transfer.cu", [f"-DGCAMB_TU_SPARSE={sp}", f"-DGCAMB_TU_NSRC={ns}"], f"transfer_s{sp}n{ns}")
     for sp in (0, 1) for ns in (2, 3)]
 NVCC_FLAGS = [

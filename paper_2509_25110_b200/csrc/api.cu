@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -49,11 +50,13 @@ static std::vector<double> trapezoid(const std::vector<double> &t)
 static void free_plan(gcamb_los_plan *p)
 {
     if (!p) return;
+    std::free(p->h_k);
     cudaFree(p->d_l_index); cudaFree(p->d_k); cudaFree(p->d_chi); cudaFree(p->d_w);
     cudaFree(p->d_dlnk); cudaFree(p->d_pref); cudaFree(p->d_start); cudaFree(p->d_tile); cudaFree(p->d_inv);
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
-    cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg);
+    cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg); cudaFree(p->d_l_user);
+    cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_cE); cudaFree(p->d_t_cB);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     if (p->h_streams_ready) {
@@ -80,6 +83,7 @@ static gcamb_status check_call(const gcamb_los_plan *p, int n_batch, const doubl
                                const double *S_E, const double *S_phi, const void *out)
 {
     if (!p || !S_T || !S_E || !out) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (p->tensor) { set_error("tensor plan: use gcamb_los_transfer_tensor / gcamb_los_cls_tensor"); return GCAMB_EINVAL; }
     if (gcamb_status st = check_device(p)) return st;
     if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
     if ((long long)p->n_k * n_batch > 0x7fffffffLL) {   // one CTA per (k, cosmology) along grid.x
@@ -108,13 +112,30 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (out) *out = nullptr;
     if (!out || !l_list || !k || !tau) { set_error("null argument"); return GCAMB_EINVAL; }
     if (n_l < 1 || n_k < 2 || n_tau < 2) { set_error("need n_l >= 1, n_k >= 2, n_tau >= 2"); return GCAMB_EINVAL; }
-    if (src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
-        set_error("src_mask must be T|E or T|E|PHI");
+    const bool tensor = src_mask == GCAMB_SRC_TENSOR;
+    if (!tensor && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
+        set_error("src_mask must be T|E, T|E|PHI or TENSOR");
         return GCAMB_EINVAL;
     }
+    const int l_top = tensor ? 65534 : 65535;   // a tensor plan also walks l + 1
     for (int i = 0; i < n_l; ++i) {
-        if (l_list[i] < 2 || l_list[i] > 65535) { set_error("l_list[%d] = %d outside [2, 65535]", i, l_list[i]); return GCAMB_EINVAL; }
+        if (l_list[i] < 2 || l_list[i] > l_top) { set_error("l_list[%d] = %d outside [2, %d]", i, l_list[i], l_top); return GCAMB_EINVAL; }
         if (i && l_list[i] <= l_list[i - 1]) { set_error("l_list not strictly increasing at %d", i); return GCAMB_EINVAL; }
+    }
+    // Tensor plans (tensor.cu): the E and B kernels need j_{l+1} next to j_l, so the kernels run on the
+    // union of {l} and {l + 1}; the caller's list and the positions of l and l + 1 in the union are kept.
+    const int32_t *user_list = l_list;
+    const int32_t n_user = n_l;
+    std::vector<int32_t> ext, pos0, pos1;
+    if (tensor) {
+        for (int i = 0; i < n_l; ++i) {
+            if (ext.empty() || ext.back() != l_list[i]) ext.push_back(l_list[i]);
+            pos0.push_back((int32_t)ext.size() - 1);
+            ext.push_back(l_list[i] + 1);
+            pos1.push_back((int32_t)ext.size() - 1);
+        }
+        l_list = ext.data();
+        n_l = (int32_t)ext.size();
     }
     if (!std::isfinite(tau0)) { set_error("tau0 not finite"); return GCAMB_EGRID; }
     for (int j = 0; j < n_k; ++j) {
@@ -130,11 +151,16 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (!p) { set_error("out of host memory"); return GCAMB_EALLOC; }
     std::memset(p, 0, sizeof(*p));
     p->n_l = n_l; p->n_k = n_k; p->n_tau = n_tau;
+    p->n_l_out = n_user;
+    p->tensor = tensor;
     p->src_mask = src_mask;
-    p->n_src = (src_mask & GCAMB_SRC_PHI) ? 3 : 2;
+    p->n_src = (tensor || (src_mask & GCAMB_SRC_PHI)) ? 3 : 2;
     p->n_spec = p->n_src + 1;
     p->l_min = l_list[0]; p->l_max = l_list[n_l - 1];
     p->tau0 = tau0;
+    p->h_k = (double *)std::malloc(sizeof(double) * n_k);
+    if (!p->h_k) { set_error("out of host memory"); free_plan(p); return GCAMB_EALLOC; }
+    std::memcpy(p->h_k, k, sizeof(double) * n_k);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaGetDevice(&p->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
@@ -156,6 +182,20 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
 
     e = upload(&p->d_l_index, l_index, stream);
     if (e == cudaSuccess) e = upload(&p->d_l_list, std::vector<int32_t>(l_list, l_list + n_l), stream);
+    if (e == cudaSuccess) e = upload(&p->d_l_user, std::vector<int32_t>(user_list, user_list + n_user), stream);
+    if (tensor) {
+        // combination coefficients of tensor.cu: (l+1)(l+2)/sqrt((l+2)(l+1)l(l-1)) and 2(l+2)
+        std::vector<double> cE(n_user), cB(n_user);
+        for (int i = 0; i < n_user; ++i) {
+            const double l = user_list[i];
+            cE[i] = (l + 1.0) * (l + 2.0) / std::sqrt((l + 2.0) * (l + 1.0) * l * (l - 1.0));
+            cB[i] = 2.0 * (l + 2.0);
+        }
+        if (e == cudaSuccess) e = upload(&p->d_t_pos0, pos0, stream);
+        if (e == cudaSuccess) e = upload(&p->d_t_pos1, pos1, stream);
+        if (e == cudaSuccess) e = upload(&p->d_t_cE, cE, stream);
+        if (e == cudaSuccess) e = upload(&p->d_t_cB, cB, stream);
+    }
     {   // sparse l lists: which tiles hold a listed l (NULL table = all of them)
         std::vector<uint32_t> mask((p->n_tiles + 31) / 32, 0u);
         for (int i = 0; i < n_l; ++i) {
@@ -181,7 +221,7 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (e != cudaSuccess) { gcamb_status st = cuda_fail(e, "plan tables"); free_plan(p); return st; }
 
     gcamb_status st = plan_precompute(p, stream);
-    if (st == GCAMB_OK) st = interp_plan_tables(p, l_list, stream);
+    if (st == GCAMB_OK) st = interp_plan_tables(p, user_list, stream);
     if (st != GCAMB_OK) { free_plan(p); return st; }
     *out = p;
     return GCAMB_OK;
@@ -206,7 +246,7 @@ gcamb_status gcamb_los_plan_info(const gcamb_los_plan *plan, int32_t *n_l, int32
                                  int32_t *n_src, int32_t *n_spec, int64_t *executed_terms)
 {
     if (!plan) { set_error("null plan"); return GCAMB_EINVAL; }
-    if (n_l) *n_l = plan->n_l;
+    if (n_l) *n_l = plan->n_l_out;
     if (n_k) *n_k = plan->n_k;
     if (n_tau) *n_tau = plan->n_tau;
     if (n_src) *n_src = plan->n_src;
@@ -242,6 +282,7 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch, 
                                    const double *d_P_R, double *d_Cl, void *cuda_stream)
 {
     if (!plan || !d_Delta || !d_P_R || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (plan->tensor) { set_error("tensor plan: use gcamb_los_cls_tensor"); return GCAMB_EINVAL; }
     if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
     if (gcamb_status st = check_device(plan)) return st;
     return launch_cls(plan, n_batch, d_Delta, d_P_R, d_Cl, (cudaStream_t)cuda_stream);
@@ -251,6 +292,33 @@ gcamb_status gcamb_los_cls(const gcamb_los_plan *plan, const double *d_Delta, co
                            double *d_Cl, void *cuda_stream)
 {
     return gcamb_los_cls_batched(plan, 1, d_Delta, d_P_R, d_Cl, cuda_stream);
+}
+
+gcamb_status gcamb_los_tensor_work_bytes(const gcamb_los_plan *plan, int64_t *bytes)
+{
+    if (!plan || !bytes) { set_error("null argument"); return GCAMB_EINVAL; }
+    if (!plan->tensor) { set_error("not a tensor plan"); return GCAMB_EINVAL; }
+    *bytes = (int64_t)tensor_work_bytes(plan);
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_transfer_tensor(const gcamb_los_plan *plan, const double *d_S_T, const double *d_S_E,
+                                       const double *d_S_B, double *d_Delta, double *d_work, void *cuda_stream)
+{
+    if (!plan || !d_S_T || !d_S_E || !d_S_B || !d_Delta || !d_work) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (!plan->tensor) { set_error("not a tensor plan (create it with GCAMB_SRC_TENSOR)"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(plan)) return st;
+    return launch_transfer_tensor(plan, d_S_T, d_S_E, d_S_B, d_Delta, d_work, (cudaStream_t)cuda_stream);
+}
+
+gcamb_status gcamb_los_cls_tensor(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_t,
+                                  double *d_Cl, void *cuda_stream)
+{
+    if (!plan || !d_Delta || !d_P_t || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (!plan->tensor) { set_error("not a tensor plan (create it with GCAMB_SRC_TENSOR)"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(plan)) return st;
+    // Eq. 1 on (T, E, B): the scalar kernels' (TT, EE, TE, third-source auto) written in the order TT, EE, BB, TE
+    return launch_cls(plan, 1, d_Delta, d_P_t, d_Cl, (cudaStream_t)cuda_stream);
 }
 
 gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Cl,

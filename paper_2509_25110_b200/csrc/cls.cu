@@ -35,7 +35,7 @@ template <int NSRC, int R, int VEC, int CLS_THREADS>
 __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restrict__ Delta,
                                                           const double *__restrict__ P_R,
                                                           const double *__restrict__ dlnk,
-                                                          double *__restrict__ Cl, int n_l, int n_k)
+                                                          double *__restrict__ Cl, int n_l, int n_k, int te_last)
 {
     constexpr int NSPEC = NSRC + 1;
     using pack = Pack<VEC>;
@@ -98,7 +98,8 @@ __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restri
             double v = 0.0;
 #pragma unroll
             for (int wv = 0; wv < CLS_THREADS / 32; ++wv) v += sm[threadIdx.x][wv];
-            Cl[((size_t)b * NSPEC + q) * n_l + l0 + r] = 4.0 * 3.14159265358979323846 * v;
+            const int q_out = (te_last && q >= 2) ? 5 - q : q;     // tensor plans: (TT, EE, BB, TE)
+            Cl[((size_t)b * NSPEC + q_out) * n_l + l0 + r] = 4.0 * 3.14159265358979323846 * v;
         }
     }
 }
@@ -126,7 +127,7 @@ __global__ void __launch_bounds__(CLS_CONSUMERS + 32, 1) cls_stream_kernel(const
                                                                            const double *__restrict__ P_R,
                                                                            const double *__restrict__ dlnk,
                                                                            double *__restrict__ Cl, int n_l, int n_k,
-                                                                           long long n_rows, int KC, int n_chunks)
+                                                                           long long n_rows, int KC, int n_chunks, int te_last)
 {
     constexpr int NSPEC = NSRC + 1, NW = CLS_CONSUMERS / 32;
     extern __shared__ __align__(16) double sm_cls[];
@@ -222,7 +223,9 @@ __global__ void __launch_bounds__(CLS_CONSUMERS + 32, 1) cls_stream_kernel(const
 #pragma unroll
             for (int wv = 0; wv < NW; ++wv) v += ps[tid * NW + wv];
             const long long li = row - b * n_l;
-            Cl[((size_t)b * NSPEC + tid) * n_l + li] = 4.0 * 3.14159265358979323846 * v;
+            // tensor plans write (TT, EE, BB, TE): the cross spectrum last
+            const int q_out = (te_last && tid >= 2) ? 5 - tid : tid;
+            Cl[((size_t)b * NSPEC + q_out) * n_l + li] = 4.0 * 3.14159265358979323846 * v;
         }
     }
 }
@@ -235,10 +238,10 @@ static size_t cls_stream_smem(int n_src, int n_k, int KC)
 
 template <int NSRC, int R, int THREADS>
 static void launch_rows(bool vec, dim3 grid, cudaStream_t stream, const double *Delta, const double *P_R,
-                        const double *dlnk, double *Cl, int n_l, int n_k)
+                        const double *dlnk, double *Cl, int n_l, int n_k, int te_last)
 {
-    if (vec) cls_kernel<NSRC, R, 2, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
-    else cls_kernel<NSRC, R, 1, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k);
+    if (vec) cls_kernel<NSRC, R, 2, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k, te_last);
+    else cls_kernel<NSRC, R, 1, THREADS><<<grid, THREADS, 0, stream>>>(Delta, P_R, dlnk, Cl, n_l, n_k, te_last);
 }
 
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,
@@ -249,7 +252,7 @@ gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delt
     if (p->n_k % 2 == 0 && (uintptr_t)Delta % 16 == 0 && p->n_k <= CLS_STREAM_MAX_K) {
         const int n_chunks = (p->n_k + CLS_STREAM_CHUNK - 1) / CLS_STREAM_CHUNK;
         const int KC = (((p->n_k + n_chunks - 1) / n_chunks) + 1) & ~1;      // even: every chunk starts 16-byte aligned
-        const long long n_rows = (long long)n_batch * p->n_l;
+        const long long n_rows = (long long)n_batch * p->n_l_out;
         const unsigned grid = (unsigned)std::min<long long>(n_rows, p->n_sm);
         const size_t smem = cls_stream_smem(p->n_src, p->n_k, KC);
         auto kern = p->n_src == 2 ? cls_stream_kernel<2> : cls_stream_kernel<3>;
@@ -260,15 +263,15 @@ gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delt
                                             (int)cls_stream_smem(p->n_src, CLS_STREAM_MAX_K, CLS_STREAM_CHUNK)));
             attr_done[p->n_src - 2].fetch_or(dev_bit, std::memory_order_release);
         }
-        kern<<<grid, CLS_CONSUMERS + 32, smem, stream>>>(Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k, n_rows, KC, n_chunks);
+        kern<<<grid, CLS_CONSUMERS + 32, smem, stream>>>(Delta, P_R, p->d_dlnk, Cl, p->n_l_out, p->n_k, n_rows, KC, n_chunks, p->tensor);
         GCAMB_CUDA(cudaGetLastError());
         return GCAMB_OK;
     }
     int R = CLS_ROWS, threads = CLS_THREADS_DEFAULT;
     // few rows: one row per CTA keeps more SMs busy
-    while (R > 1 && (long long)((p->n_l + R - 1) / R) * n_batch < 2LL * p->n_sm) R >>= 1;
-    dim3 grid((unsigned)((p->n_l + R - 1) / R), (unsigned)n_batch);
-#define GCAMB_CLS(NS, RR, TH) launch_rows<NS, RR, TH>(vec, grid, stream, Delta, P_R, p->d_dlnk, Cl, p->n_l, p->n_k)
+    while (R > 1 && (long long)((p->n_l_out + R - 1) / R) * n_batch < 2LL * p->n_sm) R >>= 1;
+    dim3 grid((unsigned)((p->n_l_out + R - 1) / R), (unsigned)n_batch);
+#define GCAMB_CLS(NS, RR, TH) launch_rows<NS, RR, TH>(vec, grid, stream, Delta, P_R, p->d_dlnk, Cl, p->n_l_out, p->n_k, p->tensor)
 #define GCAMB_CLS_R(NS, TH) do { if (R == 4) GCAMB_CLS(NS, 4, TH); else if (R == 2) GCAMB_CLS(NS, 2, TH); else GCAMB_CLS(NS, 1, TH); } while (0)
     if (p->n_src == 2) { if (threads == 128) GCAMB_CLS_R(2, 128); else GCAMB_CLS_R(2, 256); }
     else               { if (threads == 128) GCAMB_CLS_R(3, 128); else GCAMB_CLS_R(3, 256); }

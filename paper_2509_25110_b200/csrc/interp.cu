@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(INTERP_THREADS) cl_interp_kernel(const double 
 // Plan tables of the spline (host, fp64; the matrix depends on the l list only).
 gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaStream_t stream)
 {
-    const int n = p->n_l;
+    const int n = p->n_l_out;
     if (n < 2) return GCAMB_OK;             // a single multipole cannot be interpolated: the call reports it
     std::vector<double> mult(n, 0.0), inv_diag(n, 0.0), diag(n, 0.0);
     for (int i = 1; i < n - 1; ++i)
@@ -93,11 +93,11 @@ gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaSt
         diag[i] -= mult[i] * sub;
     }
     for (int i = 1; i < n - 1; ++i) inv_diag[i] = 1.0 / diag[i];
-    const int n_all = p->l_max - p->l_min + 1;
+    const int n_all = l_list[n - 1] - l_list[0] + 1;   // tensor plans: l_max also counts l + 1
     std::vector<int32_t> seg(n_all);
     int s = 0;
     for (int a = 0; a < n_all; ++a) {
-        const int l = p->l_min + a;
+        const int l = l_list[0] + a;
         while (s < n - 2 && l > l_list[s + 1]) ++s;
         seg[a] = s;
     }
@@ -114,17 +114,18 @@ gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaSt
 gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double *Cl_samp, double *Cl_all,
                               cudaStream_t stream)
 {
-    if (p->n_l < 2) { set_error("interpolation in l needs at least two multipoles in the plan's l list"); return GCAMB_EINVAL; }
-    const size_t smem = sizeof(double) * 2 * (size_t)p->n_l;
+    if (p->n_l_out < 2) { set_error("interpolation in l needs at least two multipoles in the plan's l list"); return GCAMB_EINVAL; }
+    const size_t smem = sizeof(double) * 2 * (size_t)p->n_l_out;
     if (smem > INTERP_SMEM_MAX) {
-        set_error("interpolation in l: n_l = %d exceeds %d knots", p->n_l, (int)(INTERP_SMEM_MAX / 16));
+        set_error("interpolation in l: n_l = %d exceeds %d knots", p->n_l_out, (int)(INTERP_SMEM_MAX / 16));
         return GCAMB_EINVAL;
     }
     if (smem > 48 * 1024)
         GCAMB_CUDA(cudaFuncSetAttribute(cl_interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long series = (long long)n_batch * p->n_spec;
     cl_interp_kernel<<<(unsigned)series, INTERP_THREADS, smem, stream>>>(
-        Cl_samp, Cl_all, p->d_l_list, p->d_sp_seg, p->d_sp_mult, p->d_sp_inv_diag, p->n_l, p->l_max - p->l_min + 1);
+        Cl_samp, Cl_all, p->d_l_user, p->d_sp_seg, p->d_sp_mult, p->d_sp_inv_diag, p->n_l_out,
+        p->l_max - p->tensor - p->l_min + 1);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
 }

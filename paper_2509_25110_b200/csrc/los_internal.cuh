@@ -22,6 +22,8 @@ struct TransferShape {
 
 struct gcamb_los_plan {
     int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
+    int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l and l + 1)
+    int32_t tensor;          // tensor-mode plan (tensor.cu)
     uint32_t src_mask;
     double tau0;
     gcamb::TransferShape shape;
@@ -30,6 +32,8 @@ struct gcamb_los_plan {
     int64_t walked_terms;    // same with the tile-aligned start the kernel really walks
     int device;              // the device that owns the tables; every call checks it is the current one
     int n_sm;                // its SM count
+
+    double *h_k;             // HOST copy of the k grid [n_k] (srcinterp.cu builds its tables from it)
 
     // device tables
     int32_t *d_l_index;  // [l_max+1] position in l_list, or -1
@@ -60,6 +64,11 @@ struct gcamb_los_plan {
     double *d_sp_mult;       // [n_l] forward-elimination multipliers
     double *d_sp_inv_diag;   // [n_l] reciprocals of the eliminated diagonal
     int32_t *d_sp_seg;       // [l_max - l_min + 1] knot interval of every integer l
+    int32_t *d_l_user;       // [n_l_out] the caller's l list (knots of the spline)
+
+    // tensor plans: positions of l and l + 1 of the caller's list in l_list, combination coefficients
+    int32_t *d_t_pos0, *d_t_pos1;   // [n_l_out]
+    double *d_t_cE, *d_t_cB;        // [n_l_out] (l+1)(l+2)/sqrt((l+2)(l+1)l(l-1)),  2(l+2)
 
     // scratch of gcamb_los_spectra_host (lazily allocated)
     cudaStream_t h_copy, h_comp[4];
@@ -112,7 +121,12 @@ gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaSt
 gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double *Cl_samp, double *Cl_all,
                               cudaStream_t stream);
 
-// cls.cu
+// tensor.cu: tensor-mode transfer functions from two runs of the three-source transfer kernels
+size_t tensor_work_bytes(const gcamb_los_plan *p);
+gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, const double *S_T, const double *S_E, const double *S_B,
+                                    double *Delta, double *work, cudaStream_t stream);
+
+// cls.cu (tensor plans: rows of n_l_out multipoles, spectra written in the order TT, EE, BB, TE)
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,
                         const double *P_R, double *Cl, cudaStream_t stream);
 

@@ -15,7 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgcamb_los.so")
 
-GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI = 1, 2, 4
+GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI, GCAMB_SRC_TENSOR = 1, 2, 4, 8
 _STATUS = {0: "GCAMB_OK", 1: "GCAMB_EINVAL", 2: "GCAMB_EGRID", 3: "GCAMB_EALLOC", 4: "GCAMB_ECUDA"}
 
 EXPORTS = (
@@ -23,6 +23,8 @@ EXPORTS = (
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
     "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
+    "gcamb_los_tensor_work_bytes", "gcamb_los_transfer_tensor", "gcamb_los_cls_tensor",
+    "gcamb_los_srcinterp_create", "gcamb_los_srcinterp_destroy", "gcamb_los_interp_sources",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
 PROBE_LIB_PATH = os.path.join(_HERE, "libgcamb_probe.so")
@@ -62,6 +64,12 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_spectra_batched_info.argtypes = [_vp, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32),
                                                    ctypes.POINTER(_i64)]
     lib.gcamb_los_cl_interp.argtypes = [_vp, _i32, _vp, _vp, _vp]
+    lib.gcamb_los_tensor_work_bytes.argtypes = [_vp, ctypes.POINTER(_i64)]
+    lib.gcamb_los_transfer_tensor.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_cls_tensor.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_srcinterp_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _i32, _vp]
+    lib.gcamb_los_srcinterp_destroy.argtypes = [_vp]
+    lib.gcamb_los_interp_sources.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     _lib = lib
     return lib
 
@@ -100,14 +108,15 @@ def _host(a, shape, name: str) -> np.ndarray | None:
 class Plan:
     """gcamb_los_plan: grids, quadrature weights and recurrence start values on the device."""
 
-    def __init__(self, l_list, k, tau, tau0: float, with_phi: bool = False):
+    def __init__(self, l_list, k, tau, tau0: float, with_phi: bool = False, tensor: bool = False):
         if not torch.cuda.is_available():
             raise RuntimeError("gcamb_los needs a CUDA device (no CPU fallback)")
         lib = load_library()
         l_list = np.ascontiguousarray(l_list, dtype=np.int32)
         k = np.ascontiguousarray(k, dtype=np.float64)
         tau = np.ascontiguousarray(tau, dtype=np.float64)
-        mask = GCAMB_SRC_T | GCAMB_SRC_E | (GCAMB_SRC_PHI if with_phi else 0)
+        mask = GCAMB_SRC_TENSOR if tensor else GCAMB_SRC_T | GCAMB_SRC_E | (GCAMB_SRC_PHI if with_phi else 0)
+        self.tensor = bool(tensor)
         handle = _vp()
         _check(lib.gcamb_los_plan_create(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
                                          k.ctypes.data, k.size, tau.ctypes.data, tau.size,
@@ -172,6 +181,34 @@ class Plan:
             _check(lib.gcamb_los_cls(self._h, pD, pP, pC, _stream()))
         return out
 
+    # ---- tensor modes (plans created with tensor=True)
+    def gcamb_los_tensor_work_bytes(self) -> int:
+        n = _i64()
+        _check(load_library().gcamb_los_tensor_work_bytes(self._h, ctypes.byref(n)))
+        return n.value
+
+    def gcamb_los_transfer_tensor(self, S_T, S_E, S_B, out=None, work=None) -> torch.Tensor:
+        """Tensor sources [n_k][n_tau] x 3 -> Delta [3][n_l][n_k] (T, E, B)."""
+        sh = (self.n_k, self.n_tau)
+        if out is None:
+            out = torch.empty((3, self.n_l, self.n_k), dtype=torch.float64, device=S_T.device)
+        n_work = self.gcamb_los_tensor_work_bytes() // 8
+        if work is None:
+            work = torch.empty(n_work, dtype=torch.float64, device=S_T.device)
+        _check(load_library().gcamb_los_transfer_tensor(
+            self._h, _dev(S_T, sh, "S_T"), _dev(S_E, sh, "S_E"), _dev(S_B, sh, "S_B"),
+            _dev(out, (3, self.n_l, self.n_k), "Delta"), _dev(work, (n_work,), "work"), _stream()))
+        return out
+
+    def gcamb_los_cls_tensor(self, Delta, P_t, out=None) -> torch.Tensor:
+        """Delta [3][n_l][n_k] -> C_l [4][n_l] (TT, EE, BB, TE)."""
+        if out is None:
+            out = torch.empty((4, self.n_l), dtype=torch.float64, device=Delta.device)
+        _check(load_library().gcamb_los_cls_tensor(
+            self._h, _dev(Delta, (3, self.n_l, self.n_k), "Delta"), _dev(P_t, (self.n_k,), "P_t"),
+            _dev(out, (4, self.n_l), "Cl"), _stream()))
+        return out
+
     def gcamb_los_cl_interp(self, Cl, out=None) -> torch.Tensor:
         """C_l on the l list [..., n_spec, n_l] -> C_l on every integer l [..., n_spec, l_last - l_first + 1]."""
         lead = tuple(Cl.shape[:-2])
@@ -213,8 +250,45 @@ class Plan:
             aR.ctypes.data, aC.ctypes.data, None if aD is None else aD.ctypes.data, _stream()))
 
 
-def gcamb_los_plan_create(l_list, k, tau, tau0, with_phi=False) -> Plan:
-    return Plan(l_list, k, tau, tau0, with_phi)
+def gcamb_los_plan_create(l_list, k, tau, tau0, with_phi=False, tensor=False) -> Plan:
+    return Plan(l_list, k, tau, tau0, with_phi, tensor)
+
+
+class SourceInterp:
+    """gcamb_los_srcinterp: sources on a coarse k grid -> sources on the plan's k grid (InterpolateSources)."""
+
+    def __init__(self, plan: Plan, k_coarse):
+        k_coarse = np.ascontiguousarray(k_coarse, dtype=np.float64)
+        handle = _vp()
+        _check(load_library().gcamb_los_srcinterp_create(ctypes.byref(handle), plan._h, k_coarse.ctypes.data,
+                                                         k_coarse.size, _stream()))
+        self._h = handle
+        self.n_kc, self.n_k, self.n_tau = int(k_coarse.size), plan.n_k, plan.n_tau
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            _check(load_library().gcamb_los_srcinterp_destroy(self._h))
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def gcamb_los_interp_sources(self, S_coarse, out=None, work=None) -> torch.Tensor:
+        """[..., n_kc, n_tau] -> [..., n_k, n_tau]; the leading dimensions are independent series."""
+        lead = tuple(S_coarse.shape[:-2])
+        n_series = int(np.prod(lead)) if lead else 1
+        if out is None:
+            out = torch.empty(lead + (self.n_k, self.n_tau), dtype=torch.float64, device=S_coarse.device)
+        if work is None:
+            work = torch.empty_like(S_coarse)
+        _check(load_library().gcamb_los_interp_sources(
+            self._h, n_series, _dev(S_coarse, lead + (self.n_kc, self.n_tau), "S_coarse"),
+            _dev(out, lead + (self.n_k, self.n_tau), "S_fine"), _dev(work, lead + (self.n_kc, self.n_tau), "work"),
+            _stream()))
+        return out
 
 
 _probe_lib = None
