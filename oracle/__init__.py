@@ -60,6 +60,12 @@ def _lib(real: str) -> ctypes.CDLL:
             lib.oracle_transfer_tensor.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
                                                    ctypes.c_double, _pd, _pd, _pd, ctypes.c_int, ctypes.c_int, _pd]
             lib.oracle_cls_tensor.argtypes = [ctypes.c_int, _pd, ctypes.c_int, _pd, _pd, ctypes.c_int, _pd]
+            lib.oracle_hyp_lcut_open.argtypes = [ctypes.c_double, ctypes.c_double]
+            lib.oracle_hyp_lcut_open.restype = ctypes.c_int
+            lib.oracle_hyp_bessel_open.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_transfer_open.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
+                                                 ctypes.c_double, ctypes.c_double, _pd, _pd, _pd, ctypes.c_int,
+                                                 ctypes.c_int, _pd]
             lib.oracle_interp_sources.argtypes = [_pd, ctypes.c_int, _pd, ctypes.c_int, ctypes.c_int, _pd, _pd]
             assert lib.oracle_real_mant_bits() == (53 if real == "f64" else 64)
             _LIBS[real] = lib
@@ -189,4 +195,35 @@ def interp_sources(k_coarse, k, S_coarse, real: str = "f64") -> np.ndarray:
     rc = _lib(real).oracle_interp_sources(_ptr(k_coarse), n_kc, _ptr(k), k.size, n_tau, _ptr(S_coarse), _ptr(out))
     if rc:
         raise ValueError(f"oracle_interp_sources failed ({rc})")
+    return out
+
+
+def hyp_lcut_open(beta: float, chi: float) -> int:
+    return _lib("f64").oracle_hyp_lcut_open(float(beta), float(chi))
+
+
+def hyp_bessel_open(beta: float, chi: float, lmax: int, margin: int = DEFAULT_MARGIN, real: str = "f64") -> np.ndarray:
+    """Hyperspherical Bessel functions of an open universe Phi_l^beta(chi), l = 0..lmax (reading R28)."""
+    out = np.empty(lmax + 1, dtype=np.float64)
+    if _lib(real).oracle_hyp_bessel_open(float(beta), float(chi), int(lmax), int(margin), _ptr(out)):
+        raise ValueError("oracle_hyp_bessel_open: bad arguments")
+    return out
+
+
+def transfer_open(l_list, k, tau, tau0, curv_K, S_T, S_E, S_phi=None, margin: int = DEFAULT_MARGIN,
+                  real: str = "f64", nthreads: int = 0) -> np.ndarray:
+    """Delta[n_src][n_l][n_k] in an open universe of curvature curv_K < 0 (reading R28)."""
+    l_list = np.ascontiguousarray(l_list, dtype=np.int32)
+    k, tau, S_T, S_E = _f64(k), _f64(tau), _f64(S_T), _f64(S_E)
+    assert S_T.shape == (k.size, tau.size) and S_E.shape == S_T.shape
+    sp = None
+    if S_phi is not None:
+        S_phi = _f64(S_phi)
+        sp = _ptr(S_phi)
+    out = np.empty((3 if S_phi is not None else 2, l_list.size, k.size), dtype=np.float64)
+    rc = _lib(real).oracle_transfer_open(l_list.ctypes.data_as(_pi), l_list.size, _ptr(k), k.size, _ptr(tau),
+                                         tau.size, float(tau0), float(curv_K), _ptr(S_T), _ptr(S_E), sp,
+                                         int(margin), int(nthreads), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_transfer_open failed ({rc})")
     return out
