@@ -56,6 +56,7 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
     cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg); cudaFree(p->d_l_user);
+    cudaFree(p->d_cth); cudaFree(p->d_s2); cudaFree(p->d_ib2); cudaFree(p->d_coef);
     cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_cE); cudaFree(p->d_t_cB);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
@@ -105,14 +106,23 @@ extern "C" {
 
 const char *gcamb_los_last_error(void) { return g_err; }
 
-gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
-                                   const double *k, int32_t n_k, const double *tau, int32_t n_tau,
-                                   double tau0, uint32_t src_mask, void *cuda_stream)
+}  // extern "C"
+
+// curv_K = 0: flat; curv_K < 0: open universe (reading R28)
+static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
+                                const double *k, int32_t n_k, const double *tau, int32_t n_tau,
+                                double tau0, double curv_K, uint32_t src_mask, void *cuda_stream)
 {
     if (out) *out = nullptr;
     if (!out || !l_list || !k || !tau) { set_error("null argument"); return GCAMB_EINVAL; }
     if (n_l < 1 || n_k < 2 || n_tau < 2) { set_error("need n_l >= 1, n_k >= 2, n_tau >= 2"); return GCAMB_EINVAL; }
+    const bool curved = curv_K != 0.0;
+    if (curved && !(curv_K < 0.0 && std::isfinite(curv_K))) {
+        set_error("curvature K must be negative and finite: closed universes (integer beta) are not built");
+        return GCAMB_EINVAL;
+    }
     const bool tensor = src_mask == GCAMB_SRC_TENSOR;
+    if (curved && tensor) { set_error("tensor plans are flat only"); return GCAMB_EINVAL; }
     if (!tensor && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
         set_error("src_mask must be T|E, T|E|PHI or TENSOR");
         return GCAMB_EINVAL;
@@ -153,6 +163,8 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     p->n_l = n_l; p->n_k = n_k; p->n_tau = n_tau;
     p->n_l_out = n_user;
     p->tensor = tensor;
+    p->curved = curved;
+    p->r_c = curved ? 1.0 / std::sqrt(-curv_K) : 0.0;
     p->src_mask = src_mask;
     p->n_src = (tensor || (src_mask & GCAMB_SRC_PHI)) ? 3 : 2;
     p->n_spec = p->n_src + 1;
@@ -171,6 +183,18 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     // IntegrationVars_init: the O(N) tables, on the host in fp64
     std::vector<double> vk(k, k + n_k), vtau(tau, tau + n_tau), chi(n_tau), lnk(n_k), pref(n_l);
     for (int i = 0; i < n_tau; ++i) chi[i] = tau0 - tau[i];
+    std::vector<double> cth, s2, ib2;
+    if (curved) {   // chi_i = sqrt(-K) (tau0 - tau_i), one rounding, like the flat x = k chi; beta_j = k_j r_c
+        const double sk = std::sqrt(-curv_K);
+        cth.resize(n_tau); s2.resize(n_tau); ib2.resize(n_k);
+        for (int i = 0; i < n_tau; ++i) {
+            chi[i] = sk * (tau0 - tau[i]);
+            const double sh = std::sinh(chi[i]);
+            cth[i] = std::cosh(chi[i]) / sh;
+            s2[i] = 1.0 / (sh * sh);
+        }
+        for (int j = 0; j < n_k; ++j) { const double beta = k[j] * p->r_c; ib2[j] = 1.0 / (beta * beta); }
+    }
     for (int j = 0; j < n_k; ++j) lnk[j] = std::log(k[j]);
     std::vector<double> w = trapezoid(vtau), dlnk = trapezoid(lnk);
     std::vector<int32_t> l_index((size_t)p->l_max + 1, -1);
@@ -214,7 +238,13 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     const size_t npt = (size_t)n_k * n_tau;
     if (e == cudaSuccess) e = cudaMalloc(&p->d_start, sizeof(double2) * npt);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_tile, sizeof(int32_t) * npt);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_inv, sizeof(double) * npt);
+    if (e == cudaSuccess && !curved) e = cudaMalloc(&p->d_inv, sizeof(double) * npt);
+    if (curved) {
+        if (e == cudaSuccess) e = upload(&p->d_cth, cth, stream);
+        if (e == cudaSuccess) e = upload(&p->d_s2, s2, stream);
+        if (e == cudaSuccess) e = upload(&p->d_ib2, ib2, stream);
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_coef, sizeof(double2) * (size_t)n_k * p->n_tiles * p->shape.V);
+    }
     if (e == cudaSuccess) e = cudaMalloc(&p->d_korder, sizeof(int32_t) * n_k);
     // the uploads read pageable vectors that die with this scope
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -225,6 +255,27 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     if (st != GCAMB_OK) { free_plan(p); return st; }
     *out = p;
     return GCAMB_OK;
+}
+
+extern "C" {
+
+gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
+                                   const double *k, int32_t n_k, const double *tau, int32_t n_tau,
+                                   double tau0, uint32_t src_mask, void *cuda_stream)
+{
+    return create_plan(out, l_list, n_l, k, n_k, tau, n_tau, tau0, 0.0, src_mask, cuda_stream);
+}
+
+gcamb_status gcamb_los_plan_create_open(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
+                                        const double *k, int32_t n_k, const double *tau, int32_t n_tau,
+                                        double tau0, double curvature_K, uint32_t src_mask, void *cuda_stream)
+{
+    if (!(curvature_K < 0.0)) {
+        if (out) *out = nullptr;
+        set_error("gcamb_los_plan_create_open needs K < 0 (K = 0: gcamb_los_plan_create; K > 0 is not built)");
+        return GCAMB_EINVAL;
+    }
+    return create_plan(out, l_list, n_l, k, n_k, tau, n_tau, tau0, curvature_K, src_mask, cuda_stream);
 }
 
 gcamb_status gcamb_los_plan_destroy(gcamb_los_plan *plan)

@@ -332,7 +332,7 @@ constexpr int FUSED_T_MAX_NB2 = 5, FUSED_T_MAX_NB1 = 10;
 
 bool fused_supported(const gcamb_los_plan *p, int n_batch)
 {
-    return p->n_src == 2 && n_batch >= 2 && p->n_tau <= F_THREADS * FUSED_T_MAX_NB1;
+    return p->n_src == 2 && !p->curved && n_batch >= 2 && p->n_tau <= F_THREADS * FUSED_T_MAX_NB1;
 }
 
 int fused_block(const gcamb_los_plan *p, int n_batch)

@@ -24,6 +24,8 @@ struct gcamb_los_plan {
     int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
     int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l and l + 1)
     int32_t tensor;          // tensor-mode plan (tensor.cu)
+    int32_t curved;          // open-universe plan (reading R28): hyperspherical Bessel functions
+    double r_c;              // curvature radius 1/sqrt(-K) (curved plans)
     uint32_t src_mask;
     double tau0;
     gcamb::TransferShape shape;
@@ -65,6 +67,12 @@ struct gcamb_los_plan {
     double *d_sp_inv_diag;   // [n_l] reciprocals of the eliminated diagonal
     int32_t *d_sp_seg;       // [l_max - l_min + 1] knot interval of every integer l
     int32_t *d_l_user;       // [n_l_out] the caller's l list (knots of the spline)
+
+    // open-universe plans: d_chi holds chi_i = (tau0 - tau_i)/r_c; d_inv is not allocated
+    double *d_cth;           // [n_tau] coth(chi_i)
+    double *d_s2;            // [n_tau] 1/sinh^2(chi_i)
+    double *d_ib2;           // [n_k]   1/beta_j^2, beta_j = k_j r_c
+    double2 *d_coef;         // [n_k][n_tiles V] (A_l, R_l) = ((2l+1)/b_l, b_{l+1}/b_l), l = l_max - index
 
     // tensor plans: positions of l and l + 1 of the caller's list in l_list, combination coefficients
     int32_t *d_t_pos0, *d_t_pos1;   // [n_l_out]

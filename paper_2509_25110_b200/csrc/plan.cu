@@ -37,30 +37,67 @@ __device__ __forceinline__ double j1_series(double x)
     return sum;
 }
 
+// Open universe (nonflat, reading R28): the radial functions are the hyperspherical Bessel functions
+// Phi_l^beta(chi), beta = k r_c, chi = (tau0 - tau)/r_c, with
+//   b_{l+1} Phi_{l+1} = (2l+1) coth(chi) Phi_l - b_l Phi_{l-1},   b_l = sqrt(beta^2 + l^2).
+// Above the turning point l + 1/2 = beta sinh(chi) the regular solution falls by the smaller root r_l of
+// b_{l+1} r^2 - (2l+1) coth(chi) r + b_l = 0 per step (-> tanh(chi/2) for l >> beta, slower than the flat
+// j_l when chi is not small): the cut is the first l at which the product of the r_l is below 1e-36, + 8.
+__device__ __forceinline__ int l_cut_open(double beta, double cth, double x_turn)
+{
+    int l = max(1, (int)ceil(x_turn));
+    double lg = 0.0;
+    const double b2 = beta * beta;
+    while (lg > -82.9 && l < 4000000) {
+        const double bl = sqrt(fma((double)l, (double)l, b2)), bl1 = sqrt(fma((double)(l + 1), (double)(l + 1), b2));
+        const double t = (double)(2 * l + 1) * cth;
+        const double disc = fma(t, t, -4.0 * bl * bl1);
+        if (disc > 0.0) lg += log(2.0 * bl / (t + sqrt(disc)));
+        ++l;
+    }
+    return l + 8;
+}
+
+// CURVED: `chi` holds chi_i = (tau0 - tau_i)/r_c and `k` is multiplied by r_c to give beta; inv_x is not written.
+template <bool CURVED>
 __global__ void __launch_bounds__(128) start_values_kernel(const double *__restrict__ k,
                                                            const double *__restrict__ chi, int n_tau,
-                                                           int l_max, int V,
+                                                           int l_max, int V, double r_c,
                                                            double2 *__restrict__ start,
                                                            int32_t *__restrict__ tile,
-                                                           double *__restrict__ inv_x)
+                                                           double *__restrict__ inv_x,
+                                                           int32_t *__restrict__ cut)
 {
     const int i = blockIdx.y * blockDim.x + threadIdx.x;   // k along grid.x: n_k is bounded by 2^31 - 1 only
     const int j = blockIdx.x;
     if (i >= n_tau) return;
-    const double x = __dmul_rn(k[j], chi[i]);
-    const int L = l_cut(x);
+    const double beta = CURVED ? __dmul_rn(k[j], r_c) : 0.0;
+    const double ch = chi[i];
+    const double x = CURVED ? __dmul_rn(beta, ch) : __dmul_rn(k[j], ch);
+    const double snh = CURVED ? sinh(ch) : 0.0, cth = CURVED ? cosh(ch) / snh : 0.0;
+    const int L = CURVED ? l_cut_open(beta, cth, beta * snh) : l_cut(x);
     const int Ls = min(L, l_max);
     const int t = (l_max - Ls) / V;
     const int lhi = l_max - t * V;  // Ls <= lhi < Ls + V
     const int M = max(L, lhi) + 50;
+    if (CURVED) cut[(size_t)j * n_tau + i] = Ls;
 
     double fa = 0.0, fb = 1.0;  // f_{l+1}, f_l
     double rhi = 0.0, rlo = 0.0;
     int e = 0, re = 0;
+    const double b2 = beta * beta;
+    double b_up = CURVED ? sqrt(fma((double)(M + 1), (double)(M + 1), b2)) : 0.0;   // b_{l+1}
     for (int l = M; l >= 1; --l) {
         if (l == lhi) { rlo = fb; rhi = fa; re = e; }
-        const double c = (double)(2 * l + 1) / x;
-        const double fn = fma(c, fb, -fa);
+        double fn;
+        if (CURVED) {
+            const double bl = sqrt(fma((double)l, (double)l, b2));
+            fn = ((double)(2 * l + 1) * cth * fb - b_up * fa) / bl;
+            b_up = bl;
+        } else {
+            const double c = (double)(2 * l + 1) / x;
+            fn = fma(c, fb, -fa);
+        }
         fa = fb;
         fb = fn;
         if (fabs(fb) > 0x1p500) { fa *= 0x1p-500; fb *= 0x1p-500; ++e; }
@@ -69,8 +106,17 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
     double s, c;
     sincos(x, &s, &c);
     const double inv = 1.0 / x;
-    const double j0 = s * inv;
-    const double j1 = x < 1.0 ? j1_series(x) : (s * inv - c) * inv;
+    double j0, j1;
+    if (CURVED) {
+        // Phi_0 = sin(beta chi)/(beta sinh chi), Phi_1 = (coth sin - beta cos)/(beta sinh chi b_1); for x < 1 the
+        // closed form of Phi_1 cancels and Phi_0 ~ 1 alone fixes the scale
+        const double d = 1.0 / (beta * snh);
+        j0 = s * d;
+        j1 = x < 1.0 ? fa * (j0 / fb) : (cth * s - beta * c) * d / sqrt(b2 + 1.0);
+    } else {
+        j0 = s * inv;
+        j1 = x < 1.0 ? j1_series(x) : (s * inv - c) * inv;
+    }
     const double m = fmax(fabs(fb), fabs(fa));
     const double a = fb / m, b = fa / m;
     const double sc = (j0 * a + j1 * b) / ((a * a + b * b) * m);
@@ -85,7 +131,25 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
     const size_t idx = (size_t)j * n_tau + i;
     start[idx] = out;
     tile[idx] = t;
-    inv_x[idx] = inv;   // 1/x, correctly rounded: the transfer kernel's coefficient base
+    if (!CURVED) inv_x[idx] = inv;   // 1/x, correctly rounded: the transfer kernel's coefficient base
+}
+
+// Open universe: per (k, l) the two coefficients of a downward step  Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1},
+// A_l = (2l+1)/b_l, R_l = b_{l+1}/b_l, laid out as the transfer kernel walks: [k][tile][step], l = l_max - tile V - step
+__global__ void __launch_bounds__(256) curved_coef_kernel(const double *__restrict__ k, double r_c, int l_max, int n_walk,
+                                                          double2 *__restrict__ coef)
+{
+    const int j = blockIdx.y;
+    const double beta = __dmul_rn(k[j], r_c), b2 = beta * beta;
+    for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < n_walk; a += gridDim.x * blockDim.x) {
+        const int l = l_max - a;
+        double2 c = make_double2(0.0, 0.0);
+        if (l >= 1) {
+            const double bl = sqrt(fma((double)l, (double)l, b2)), bl1 = sqrt(fma((double)(l + 1), (double)(l + 1), b2));
+            c = make_double2((double)(2 * l + 1) / bl, bl1 / bl);
+        }
+        coef[(size_t)j * n_walk + a] = c;
+    }
 }
 
 // per-k work: walked = sum_i (lhi_i - l_min + 1)+, executed = sum_i (min(L(x_i), l_max) - l_min + 1)+
@@ -93,6 +157,7 @@ __global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ 
                                                      const double *__restrict__ chi, int n_tau,
                                                      int l_min, int l_max, int V,
                                                      const int32_t *__restrict__ tile,
+                                                     const int32_t *__restrict__ cut,
                                                      long long *__restrict__ walked,
                                                      long long *__restrict__ executed,
                                                      long long *__restrict__ first_tile)
@@ -101,8 +166,7 @@ __global__ void __launch_bounds__(256) k_cost_kernel(const double *__restrict__ 
     const int j = blockIdx.x;
     long long w = 0, ex = 0;
     for (int i = threadIdx.x; i < n_tau; i += blockDim.x) {
-        const double x = __dmul_rn(k[j], chi[i]);
-        const int Ls = min(l_cut(x), l_max);
+        const int Ls = cut ? cut[(size_t)j * n_tau + i] : min(l_cut(__dmul_rn(k[j], chi[i])), l_max);
         const int lhi = l_max - tile[(size_t)j * n_tau + i] * V;
         w += max(0, lhi - l_min + 1);
         ex += max(0, Ls - l_min + 1);
@@ -124,21 +188,38 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
 {
     const int V = p->shape.V;
     dim3 grid(p->n_k, (p->n_tau + 127) / 128);
-    start_values_kernel<<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V,
-                                                  p->d_start, p->d_tile, p->d_inv);
-    GCAMB_CUDA(cudaGetLastError());
+    int32_t *d_cut = nullptr;
+    if (p->curved) {
+        GCAMB_CUDA(cudaMalloc(&d_cut, sizeof(int32_t) * (size_t)p->n_k * p->n_tau));
+        start_values_kernel<true><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, p->r_c,
+                                                            p->d_start, p->d_tile, nullptr, d_cut);
+        cudaError_t ec = cudaGetLastError();
+        if (ec == cudaSuccess) {
+            const int n_walk = p->n_tiles * V;
+            curved_coef_kernel<<<dim3((unsigned)((n_walk + 255) / 256), (unsigned)p->n_k), 256, 0, stream>>>(
+                p->d_k, p->r_c, p->l_max, n_walk, p->d_coef);
+            ec = cudaGetLastError();
+        }
+        if (ec != cudaSuccess) { cudaFree(d_cut); return cuda_fail(ec, "plan precompute (open universe)"); }
+    } else {
+        start_values_kernel<false><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, 0.0,
+                                                             p->d_start, p->d_tile, p->d_inv, nullptr);
+        GCAMB_CUDA(cudaGetLastError());
+    }
 
     long long *d_cost = nullptr;
-    GCAMB_CUDA(cudaMalloc(&d_cost, sizeof(long long) * 3 * (size_t)p->n_k));
+    cudaError_t e = cudaMalloc(&d_cost, sizeof(long long) * 3 * (size_t)p->n_k);
+    if (e != cudaSuccess) { cudaFree(d_cut); return cuda_fail(e, "plan precompute"); }
     k_cost_kernel<<<p->n_k, 256, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_min, p->l_max, V,
-                                              p->d_tile, d_cost, d_cost + p->n_k, d_cost + 2 * p->n_k);
-    cudaError_t e = cudaGetLastError();
+                                              p->d_tile, d_cut, d_cost, d_cost + p->n_k, d_cost + 2 * p->n_k);
+    e = cudaGetLastError();
     std::vector<long long> cost(3 * (size_t)p->n_k);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(cost.data(), d_cost, sizeof(long long) * cost.size(),
                             cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
     cudaFree(d_cost);
+    cudaFree(d_cut);
     if (e != cudaSuccess) return cuda_fail(e, "plan precompute");
 
     p->walked_terms = std::accumulate(cost.begin(), cost.begin() + p->n_k, 0LL);
@@ -194,7 +275,7 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
         for (int j = 0; j < p->n_k; ++j) n_comp += hk[j] * chi_max > COMP_X_MIN;
         bool prefix = true;
         for (int r = 0; r < p->n_k; ++r) prefix = prefix && ((hk[order[r]] * chi_max > COMP_X_MIN) == (r < n_comp));
-        p->n_comp = prefix ? n_comp : p->n_k;
+        p->n_comp = p->curved ? 0 : (prefix ? n_comp : p->n_k);   // the open-universe kernels have no compensated form
     }
     // zero region of Delta (R16): x grows with k, so the first tile of a k (that of tau_0, its
     // largest x) never rises with k, and the rows of tile t are exactly zero for the first kz[t]

@@ -55,6 +55,9 @@ struct TransferParams {
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
     int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
     int zero_fill;  // this launch also zeroes the skipped region of Delta (all rows of it)
+    // open-universe plans (CURVED kernels, reading R28); appended so that the flat kernels see the same layout
+    const double *cth, *s2, *ib2;   // coth(chi_i), 1/sinh^2(chi_i) [n_tau]; 1/beta_j^2 [n_k]
+    const double2 *coef;            // [n_k][n_tiles V] (A_l, R_l) of the step Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1}
 };
 
 constexpr int T_MAX = 12;      // points per thread: the NA dispatch of the kernel is written out up to 12
@@ -128,8 +131,10 @@ constexpr int LAG = 1;   // a group is flushed this many groups after it was wri
 // The compensated body adds the reciprocal's rounding residual: c = fma(2l+1, inv, e) with
 // e = (2l_top+1) * inv_lo taken once per tile (inv_lo ~ 1e-16 inv: its change inside a tile is
 // far below an ulp of c), which makes c the correctly rounded quotient.
-template <int NA, int T, int V, int NSRC, bool COMP>
-__device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], const double *ixlo, int stride,
+// CURVED (open universe, reading R28): the step is Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1} with the
+// per-(k, l) coefficients cf[s] = (A_l, R_l) of the plan and ix = coth(chi): one DMUL more per term.
+template <int NA, int T, int V, int NSRC, bool COMP, bool CURVED>
+__device__ __forceinline__ void tile_body(double tl0, const double2 (&cf)[V], const double (&ix)[T], const double *ixlo, int stride,
                                           const double (&src)[NSRC][T], double (&fa)[T], double (&fb)[T],
                                           double (&acc)[NSRC][V])
 {
@@ -139,11 +144,11 @@ __device__ __forceinline__ void tile_body(double tl0, const double (&ix)[T], con
         if (COMP) e = tl0 * ixlo[j * stride];
 #pragma unroll
         for (int s = 0; s < V; ++s) {
-            const double tl = tl0 - 2.0 * s;   // 2l+1
+            const double tl = CURVED ? cf[s].x : tl0 - 2.0 * s;   // 2l+1  (curved: (2l+1)/b_l)
             const double c = COMP ? fma(tl, ix[j], e) : tl * ix[j];
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
-            const double fn = fma(c, fb[j], -fa[j]);
+            const double fn = CURVED ? fma(c, fb[j], -(cf[s].y * fa[j])) : fma(c, fb[j], -fa[j]);
             fa[j] = fb[j];
             fb[j] = fn;
         }
@@ -179,9 +184,10 @@ __device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T]
 // MULTI: the tau range takes several passes (n_tau > threads * T).  A kernel of its own, so that the
 // single-pass kernels carry neither the pass loop nor the load-add-store of the flush (measured:
 // config 1 +4 % with a run-time pass count).
-template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE, bool MULTI>
+template <int T, int V, int NSRC, int G, int MAXTHREADS, int MINBLOCKS, bool COMP, bool SPARSE, bool MULTI, bool CURVED>
 __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const TransferParams p)
 {
+    static_assert(!(CURVED && (COMP || SPARSE)), "the open-universe kernels are dense and uncompensated");
     static_assert(T >= 1 && T <= T_MAX, "the NA dispatch below is written out for T <= 12");
     constexpr int P = NSRC * V;          // partial sums per thread and tile
     constexpr int NOUT = (G * P + MAXTHREADS - 1) / MAXTHREADS;   // flush outputs per thread (full CTA)
@@ -266,7 +272,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         const int ic = valid ? i : i_end - 1;
         const size_t sx = ((size_t)b * p.n_k + kidx) * p.n_tau + ic;
         GCAMB_ASSERT(kidx >= 0 && kidx < p.n_k && b < p.n_batch && ic >= 0 && ic < p.n_tau && krank < p.n_k);
-        const double inv = p.inv_x[row + ic];   // 1/x from the plan: no division in the per-call path
+        // 1/x from the plan: no division in the per-call path (open universe: coth(chi), a table over tau)
+        const double inv = CURVED ? p.cth[ic] : p.inv_x[row + ic];
         const double w = valid ? p.w[ic] : 0.0;
         fa[j] = fb[j] = 0.0;
         ix[j] = valid ? inv : 0.0;
@@ -278,7 +285,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         tp[j] = valid ? p.tile[row + ic] : NEVER;
         my_start[j * NT] = p.start[row + ic];   // never injected when the slot is masked (tile NEVER)
         src[0][j] = w * p.S[0][sx];
-        src[1][j] = w * p.S[1][sx] * (inv * inv);
+        src[1][j] = w * p.S[1][sx] * (CURVED ? p.ib2[kidx] * p.s2[ic] : inv * inv);   // 1/x^2 (1/(beta sinh chi)^2)
         if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
         my_tile[j * NT] = tp[j];
     }
@@ -432,7 +439,13 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             for (int q = 0; q < NSRC; ++q)
 #pragma unroll
                 for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
-#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C>(tl0, ix, my_ixlo, NT, src, fa, fb, acc); break;
+            double2 cf[V];   // open universe: the tile's V coefficient pairs (the same for every thread of the CTA)
+            if constexpr (CURVED) {
+                const double2 *cp = p.coef + ((size_t)kidx * p.n_tiles + t) * V;
+#pragma unroll
+                for (int s = 0; s < V; ++s) cf[s] = __ldg(cp + s);
+            }
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C, CURVED>(tl0, cf, ix, my_ixlo, NT, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
                 GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) \
@@ -489,7 +502,7 @@ constexpr int MINB_256 = 1;
 // The result depends on (n_tau, n_rows, n_sm) only; the order of every sum depends on the shape, so a
 // batched call and a single call agree bit for bit only when they choose the same shape:
 // choose_shape is therefore evaluated with the rows of ONE cosmology (n_k), never with n_k * n_batch.
-#if !defined(GCAMB_TU_SPARSE) || (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
+#if !defined(GCAMB_TU_SPARSE) || (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2 && !defined(GCAMB_TU_CURVED))
 TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm)
 {
     (void)n_src;
@@ -518,7 +531,7 @@ TransferShape choose_shape(int n_tau, int n_src, long long n_rows, int n_sm)
 #endif
 
 // One launch over positions [k_first, k_first + n_pos) of the cost order.
-template <int T, int V, int NSRC, bool COMP, bool SPARSE>
+template <int T, int V, int NSRC, bool COMP, bool SPARSE, bool CURVED>
 static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int k_first, int n_pos,
                                 bool zero_fill, bool overlap_previous, int device, cudaStream_t stream)
 {
@@ -536,15 +549,16 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
     };
     // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
     // are compiled for 3 co-resident CTAs per SM (168 registers) while that fits, else for 2
-    constexpr int MINB128 = 2 * (T * (3 + NSRC) + NSRC * V) > 140 ? 2 : MINB_128;
+    // (the open-universe kernels also hold the tile's 2 V coefficients: 2 CTAs)
+    constexpr int MINB128 = (CURVED || 2 * (T * (3 + NSRC) + NSRC * V) > 140) ? 2 : MINB_128;
     const bool small = sh.threads <= 128;
     // multi-pass launches always run 128 threads x T_MAX points (choose_shape): one more kernel, not 24
     const bool multi = sh.n_pass > 1;
     if (multi && !(T == T_MAX && small)) { set_error("internal: multi-pass shape %d x %d", sh.threads, T); return GCAMB_EINVAL; }
-    void (*kern)(TransferParams) = small ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, false>
-                                         : transfer_kernel<T, V, NSRC, RING_G, 256, MINB_256, COMP, SPARSE, false>;
+    void (*kern)(TransferParams) = small ? transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, false, CURVED>
+                                         : transfer_kernel<T, V, NSRC, RING_G, 256, MINB_256, COMP, SPARSE, false, CURVED>;
     if constexpr (T == T_MAX) {
-        if (multi) kern = transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, true>;
+        if (multi) kern = transfer_kernel<T, V, NSRC, RING_G, 128, MINB128, COMP, SPARSE, true, CURVED>;
     }
     // opt in to large dynamic shared memory once per kernel and device (bit d of the mask = device d done)
     static std::atomic<unsigned long long> attr_done[3];
@@ -574,24 +588,28 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
 // first because they are the heaviest rows; the plain launch follows, overlapped with it.
 // `zero_fill`: this range also zeroes the skipped region of Delta (for all rows).
 // SPARSE: the kernels that skip the accumulation on tiles without a listed l (sparse l lists).
-template <int T, int V, int NSRC, bool SPARSE>
+template <int T, int V, int NSRC, bool SPARSE, bool CURVED>
 static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
                                 bool zero_fill, int device, cudaStream_t stream)
 {
+    if constexpr (CURVED)   // one launch: the open-universe kernels have no compensated form (the plan sets n_comp = 0)
+        return launch_impl<T, V, NSRC, false, false, true>(prm, sh, pos0, pos1 - pos0, zero_fill, false, device, stream);
+    else {
     const int c0 = pos0, c1 = std::min(pos1, n_comp);   // compensated part
     const int q0 = std::max(pos0, n_comp), q1 = pos1;   // plain part
     const bool has_plain = q1 > q0;
-    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, device, stream);
+    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE, false>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, device, stream);
     if (st != GCAMB_OK) return st;
-    return launch_impl<T, V, NSRC, false, SPARSE>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, device, stream);
+    return launch_impl<T, V, NSRC, false, SPARSE, false>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, device, stream);
+    }
 }
 
-template <int V, int NSRC, bool SPARSE>
+template <int V, int NSRC, bool SPARSE, bool CURVED>
 static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,
                              bool zero_fill, int device, cudaStream_t stream)
 {
     switch (sh.T) {
-#define GCAMB_T(t) case t: return launch_pair<t, V, NSRC, SPARSE>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);
+#define GCAMB_T(t) case t: return launch_pair<t, V, NSRC, SPARSE, CURVED>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);
         GCAMB_T(1) GCAMB_T(2) GCAMB_T(3) GCAMB_T(4) GCAMB_T(5) GCAMB_T(6)
         GCAMB_T(7) GCAMB_T(8) GCAMB_T(9) GCAMB_T(10) GCAMB_T(11) GCAMB_T(12)
 #undef GCAMB_T
@@ -604,34 +622,49 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
 // so build.py compiles this file four times, once per entry below (-DGCAMB_TU_SPARSE=s
 // -DGCAMB_TU_NSRC=n), in parallel; the host-side functions live in the (0, 2) unit.  Without the
 // macros everything is one translation unit.
+// Two more units (-DGCAMB_TU_CURVED=1 -DGCAMB_TU_NSRC=n) hold the open-universe kernels (dense only: a sparse
+// l list is served by the dense kernels, which store the listed l only).
 #ifdef GCAMB_TU_SPARSE
-#define GCAMB_TU_HAS(sp, ns) ((sp) == GCAMB_TU_SPARSE && (ns) == GCAMB_TU_NSRC)
-#define GCAMB_TU_PRIMARY (GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
+#ifndef GCAMB_TU_CURVED
+#define GCAMB_TU_CURVED 0
+#endif
+#define GCAMB_TU_HAS(sp, ns) (!GCAMB_TU_CURVED && (sp) == GCAMB_TU_SPARSE && (ns) == GCAMB_TU_NSRC)
+#define GCAMB_TU_HAS_CURVED(ns) (GCAMB_TU_CURVED && (ns) == GCAMB_TU_NSRC)
+#define GCAMB_TU_PRIMARY (!GCAMB_TU_CURVED && GCAMB_TU_SPARSE == 0 && GCAMB_TU_NSRC == 2)
 #else
 #define GCAMB_TU_HAS(sp, ns) 1
+#define GCAMB_TU_HAS_CURVED(ns) 1
 #define GCAMB_TU_PRIMARY 1
 #endif
-#define GCAMB_ENTRY(name, NS, SP)                                                                             \
+#define GCAMB_ENTRY(name, NS, SP, CV)                                                                         \
     gcamb_status name(const TransferParams &prm, const TransferShape &sh, int n_comp, int pos0, int pos1,     \
                       bool zero_fill, int device, cudaStream_t stream)                                        \
     {                                                                                                         \
-        return launch_T<TILE_V, NS, SP>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);              \
+        return launch_T<TILE_V, NS, SP, CV>(prm, sh, n_comp, pos0, pos1, zero_fill, device, stream);          \
     }
 gcamb_status launch_range_dense_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_dense_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_sparse_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_sparse_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_curved_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_curved_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 #if GCAMB_TU_HAS(0, 2)
-GCAMB_ENTRY(launch_range_dense_2, 2, false)
+GCAMB_ENTRY(launch_range_dense_2, 2, false, false)
 #endif
 #if GCAMB_TU_HAS(0, 3)
-GCAMB_ENTRY(launch_range_dense_3, 3, false)
+GCAMB_ENTRY(launch_range_dense_3, 3, false, false)
 #endif
 #if GCAMB_TU_HAS(1, 2)
-GCAMB_ENTRY(launch_range_sparse_2, 2, true)
+GCAMB_ENTRY(launch_range_sparse_2, 2, true, false)
 #endif
 #if GCAMB_TU_HAS(1, 3)
-GCAMB_ENTRY(launch_range_sparse_3, 3, true)
+GCAMB_ENTRY(launch_range_sparse_3, 3, true, false)
+#endif
+#if GCAMB_TU_HAS_CURVED(2)
+GCAMB_ENTRY(launch_range_curved_2, 2, false, true)
+#endif
+#if GCAMB_TU_HAS_CURVED(3)
+GCAMB_ENTRY(launch_range_curved_3, 3, false, true)
 #endif
 
 #if GCAMB_TU_PRIMARY
@@ -660,6 +693,9 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.n_batch = n_batch; prm.n_pass = sh.n_pass; prm.pass_len = sh.pass_len;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.order_reversed = p->order_reversed;
+    prm.cth = p->d_cth; prm.s2 = p->d_s2; prm.ib2 = p->d_ib2; prm.coef = p->d_coef;
+    if (p->curved)
+        return (p->n_src == 2 ? launch_range_curved_2 : launch_range_curved_3)(prm, sh, 0, pos0, pos1, zero_fill, p->device, stream);
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
     if (p->n_src == 2)
         return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);

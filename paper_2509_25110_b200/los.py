@@ -19,7 +19,7 @@ GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI, GCAMB_SRC_TENSOR = 1, 2, 4, 8
 _STATUS = {0: "GCAMB_OK", 1: "GCAMB_EINVAL", 2: "GCAMB_EGRID", 3: "GCAMB_EALLOC", 4: "GCAMB_ECUDA"}
 
 EXPORTS = (
-    "gcamb_los_plan_create", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
+    "gcamb_los_plan_create", "gcamb_los_plan_create_open", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
     "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
@@ -52,6 +52,8 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_last_error.restype = ctypes.c_char_p
     lib.gcamb_los_plan_create.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64,
                                           ctypes.c_uint32, _vp]
+    lib.gcamb_los_plan_create_open.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64, _f64,
+                                               ctypes.c_uint32, _vp]
     lib.gcamb_los_plan_destroy.argtypes = [_vp]
     lib.gcamb_los_plan_info.argtypes = [_vp] + [ctypes.POINTER(_i32)] * 5 + [ctypes.POINTER(_i64)]
     lib.gcamb_los_plan_launches.argtypes = [_vp, ctypes.POINTER(_i32), ctypes.POINTER(_i32)]
@@ -108,7 +110,8 @@ def _host(a, shape, name: str) -> np.ndarray | None:
 class Plan:
     """gcamb_los_plan: grids, quadrature weights and recurrence start values on the device."""
 
-    def __init__(self, l_list, k, tau, tau0: float, with_phi: bool = False, tensor: bool = False):
+    def __init__(self, l_list, k, tau, tau0: float, with_phi: bool = False, tensor: bool = False,
+                 curvature_K: float = 0.0):
         if not torch.cuda.is_available():
             raise RuntimeError("gcamb_los needs a CUDA device (no CPU fallback)")
         lib = load_library()
@@ -118,9 +121,14 @@ class Plan:
         mask = GCAMB_SRC_TENSOR if tensor else GCAMB_SRC_T | GCAMB_SRC_E | (GCAMB_SRC_PHI if with_phi else 0)
         self.tensor = bool(tensor)
         handle = _vp()
-        _check(lib.gcamb_los_plan_create(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
-                                         k.ctypes.data, k.size, tau.ctypes.data, tau.size,
-                                         float(tau0), mask, _stream()))
+        if curvature_K != 0.0:      # open universe (K < 0); the library rejects K > 0
+            _check(lib.gcamb_los_plan_create_open(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
+                                                  k.ctypes.data, k.size, tau.ctypes.data, tau.size,
+                                                  float(tau0), float(curvature_K), mask, _stream()))
+        else:
+            _check(lib.gcamb_los_plan_create(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
+                                             k.ctypes.data, k.size, tau.ctypes.data, tau.size,
+                                             float(tau0), mask, _stream()))
         self._h = handle
         out = [_i32() for _ in range(5)]
         ex = _i64()
