@@ -437,6 +437,182 @@ def run_cuda(args) -> None:
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------- SURVEY 8(f) "next" rows
+def camb_like_l_list(l_min: int, l_max: int) -> np.ndarray:
+    """Every l below 40, every 10th to 200, every 50th above (CAMB's default sampling)."""
+    l = np.concatenate([np.arange(l_min, 40), np.arange(40, 200, 10), np.arange(200, l_max + 1, 50), [l_max]])
+    return np.unique(l[(l >= l_min) & (l <= l_max)]).astype(np.int32)
+
+
+def tensor_sources(k: np.ndarray, tau: np.ndarray, seed: int = synth.SEED):
+    """Seeded synthetic tensor sources (the recipe of tests/test_gpu_tensor.py)."""
+    kk, tt = k[:, None], tau[None, :]
+    g = np.exp(-((tt - 280.0) ** 2) / (2.0 * 20.0 ** 2)) / (20.0 * np.sqrt(2.0 * np.pi))
+    damp = np.exp(-((kk / 0.05) ** 2))
+    h = np.sin(kk * tt) / (kk * tt)
+    S = [g * h * damp + 0.3e-4 * np.exp(-(((tt - 10000.0) / 2500.0) ** 2)) * np.exp(-kk / 0.005),
+         g * h * damp * 0.2, g * np.cos(kk * tt) * damp * 0.15]
+    return [np.ascontiguousarray(x * (1.0 + 1e-3 * synth.uniform_pm1(seed, 500 + q, 0, x.size).reshape(x.shape)))
+            for q, x in enumerate(S)]
+
+
+def time_steps(step_fns, steps: int, warmup: int, flush):
+    """Mean CUDA-event time (ms) of each function of a step, L2 flushed before every step."""
+    import torch
+    for _ in range(warmup):
+        flush.zero_()
+        for f in step_fns:
+            f()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(step_fns) + 1)] for _ in range(steps)]
+    for s in range(steps):
+        flush.zero_()
+        ev[s][0].record()
+        for i, f in enumerate(step_fns):
+            f()
+            ev[s][i + 1].record()
+    torch.cuda.synchronize()
+    return [float(np.mean([e[i].elapsed_time(e[i + 1]) for e in ev])) for i in range(len(step_fns))]
+
+
+def run_next(args) -> None:
+    """One JSON line for a SURVEY 8(f) row: --workload sparse | tensor | open | srcinterp (single GPU)."""
+    import torch
+
+    import oracle
+    from paper_2509_25110_b200 import los
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    los.load_library()
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    cfg = synth.CONFIGS[1]
+    tau, tau0 = cfg.tau(), cfg.tau0
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    cores = host_cores()
+    oracle.build()
+    w = args.workload
+    sampler = ClockSampler(0)
+    sampler.start()
+    extra = {}
+    if w == "sparse":      # NEXT-2: CAMB's default operating mode on config-1 grids
+        k, l_list = cfg.k(), camb_like_l_list(cfg.l_min, cfg.l_max)
+        S = synth.sources(cfg)
+        plan = los.Plan(l_list, k, tau, tau0)
+        dS, dP = [to_dev(S[0]), to_dev(S[1])], to_dev(synth.primordial_power(cfg))
+        D = torch.empty((2, plan.n_l, plan.n_k), dtype=torch.float64, device=dev)
+        C = torch.empty((3, plan.n_l), dtype=torch.float64, device=dev)
+        C_all = torch.empty((3, plan.n_l_all), dtype=torch.float64, device=dev)
+        fns = [lambda: plan.gcamb_los_transfer(dS[0], dS[1], out=D), lambda: plan.gcamb_los_cls(D, dP, out=C),
+               lambda: plan.gcamb_los_cl_interp(C, out=C_all)]
+        names = ["transfer_ms", "cls_ms", "cl_interp_ms"]
+        tiles = np.unique((cfg.l_max - l_list) // 8).size / ((cfg.l_max - cfg.l_min) // 8 + 1)
+        flop_per_term = 2 * (2 + 2 * tiles)       # recurrence everywhere, accumulates on the tiles that hold a listed l
+        units = plan.n_l_all * plan.n_k * plan.n_tau
+        workload = (f"config-1 grids, CAMB-like list of {l_list.size} of {plan.n_l_all} multipoles: sparse transfer + cls + "
+                    f"spline to every l (reading R25)")
+        algorithmic = (f"{flop_per_term:.3f} flop per walked (l,k,tau): coefficient + recurrence on every l, 2 accumulates on "
+                       f"the {100 * tiles:.0f} % of l-tiles that hold a listed l")
+        ref = lambda sl: oracle.transfer(l_list, k[sl], tau, tau0, S[0][sl], S[1][sl], real="f64", nthreads=cores)
+        get_rows = lambda rows: D[:, :, rows]
+    elif w == "tensor":    # NEXT-3: l_max_tensor = 1500, k tau0 <= 3000 (PAPER.md:93), config-1 tau grid
+        k, l_list = synth.k_grid(1000, 1e-5, 3000.0 / tau0), np.arange(2, 1501, dtype=np.int32)
+        S = tensor_sources(k, tau)
+        plan = los.Plan(l_list, k, tau, tau0, tensor=True)
+        dS, dP = [to_dev(x) for x in S], to_dev(2.1e-10 * (k / 0.05) ** -0.01)
+        D = torch.empty((3, plan.n_l, plan.n_k), dtype=torch.float64, device=dev)
+        C = torch.empty((4, plan.n_l), dtype=torch.float64, device=dev)
+        work = torch.empty(plan.gcamb_los_tensor_work_bytes() // 8, dtype=torch.float64, device=dev)
+        fns = [lambda: plan.gcamb_los_transfer_tensor(*dS, out=D, work=work), lambda: plan.gcamb_los_cls_tensor(D, dP, out=C)]
+        names = ["transfer_ms", "cls_ms"]
+        flop_per_term, units = 2 * 8, plan.n_l * plan.n_k * plan.n_tau
+        workload = "tensor modes: l=2..1500, n_k=1000 log in [1e-5, 3000/tau0], config-1 tau grid (1200), sources T,E,B (reading R27)"
+        algorithmic = ("16 flop per executed (l,k,tau): coefficient + recurrence + the 6 plain sums of the T, E, B kernels; "
+                       "the path executes 20 (two runs of the three-source kernels)")
+        ref = lambda sl: oracle.transfer_tensor(l_list, k[sl], tau, tau0, S[0][sl], S[1][sl], S[2][sl], real="f64", nthreads=cores)
+        get_rows = lambda rows: D[:, :, rows]
+    elif w == "open":      # NEXT-4: config-1 grids in an open universe, r_c = 14000 Mpc
+        k, l_list, K = cfg.k(), cfg.l_list(), -1.0 / 14000.0 ** 2
+        S = synth.sources(cfg)
+        plan = los.Plan(l_list, k, tau, tau0, curvature_K=K)
+        dS, dP = [to_dev(S[0]), to_dev(S[1])], to_dev(synth.primordial_power(cfg))
+        D = torch.empty((2, plan.n_l, plan.n_k), dtype=torch.float64, device=dev)
+        C = torch.empty((3, plan.n_l), dtype=torch.float64, device=dev)
+        fns = [lambda: plan.gcamb_los_transfer(dS[0], dS[1], out=D), lambda: plan.gcamb_los_cls(D, dP, out=C)]
+        names = ["transfer_ms", "cls_ms"]
+        flop_per_term, units = 2 * 5, plan.n_l * plan.n_k * plan.n_tau
+        workload = "config-1 grids in an open universe, K = -1/(14000 Mpc)^2: hyperspherical Bessel functions (reading R28)"
+        algorithmic = "10 flop per executed (l,k,tau): A_l coth, R_l f_{l+1}, recurrence, 2 accumulates"
+        ref = lambda sl: oracle.transfer_open(l_list, k[sl], tau, tau0, K, S[0][sl], S[1][sl], real="f64", nthreads=cores)
+        get_rows = lambda rows: D[:, :, rows]
+    else:                  # srcinterp, NEXT-3: 300 evolved wavenumbers -> the 3000 of config 1, T and E
+        k, kc = cfg.k(), synth.k_grid(300, cfg.k_lo, cfg.k_hi)
+        coarse = synth.Config(9, "coarse", cfg.l_min, cfg.l_max, 300, cfg.k_lo, cfg.k_hi, cfg.n_tau_uniform, cfg.n_tau_log, False)
+        Sc = np.stack(synth.sources(coarse, noise=False)[:2])
+        plan = los.Plan(np.arange(2, 10, dtype=np.int32), k, tau, tau0)
+        si = los.SourceInterp(plan, kc)
+        dSc = to_dev(Sc)
+        out = torch.empty((2, plan.n_k, plan.n_tau), dtype=torch.float64, device=dev)
+        work = torch.empty_like(dSc)
+        fns = [lambda: si.gcamb_los_interp_sources(dSc, out=out, work=work)]
+        names = ["interp_sources_ms"]
+        workload = "InterpolateSources: 300 coarse -> 3000 fine wavenumbers of config 1, 1200 tau, sources T and E (reading R26)"
+    times = time_steps(fns, args.steps, args.warmup, flush)
+    clocks = sampler.stop()
+    t_step = sum(times) * 1e-3
+    peak_tf = n_sm * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    if w == "srcinterp":
+        # algorithmic bytes: coarse sources read once, second derivatives written and read once, fine sources written
+        n_c, n_f = int(dSc.numel()), int(out.numel())
+        bytes_alg = 8 * (3 * n_c + n_f)
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+        peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
+        value, unit, metric = n_f / t_step, "source values/s", "interpolated source values/s (InterpolateSources)"
+        roof = {"bound": "hbm", "kernel": "srcinterp_eval_kernel + srcinterp_solve_kernel", "achieved": bytes_alg / t_step / 1e9,
+                "peak": peak_gbs, "unit": "GB/s", "frac": bytes_alg / t_step / 1e9 / peak_gbs, "traffic": None,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
+                "algorithmic": f"{bytes_alg} bytes per call: 8 (3 n_coarse + n_fine) n_tau n_series"}
+        t0 = time.perf_counter()
+        ref_out = oracle.interp_sources(kc, k, Sc[0], real="f64")
+        dt = time.perf_counter() - t0
+        err = float(np.max(np.abs(out[0].cpu().numpy() - ref_out)) / np.max(np.abs(Sc[0])))
+        cpu = {"value": ref_out.size / dt, "unit": unit, "cores": 1, "kind": "oracle",
+               "sample": f"source T in full (one of two series), fp64 oracle build, {dt:.2f} s", "err_on_sample": err}
+        si.close()
+    else:
+        executed = plan.executed_terms
+        value, unit, metric = units / t_step, UNIT, "LOS (l,k,tau) terms/s"
+        achieved = executed * flop_per_term / (times[0] * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "transfer_kernel", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": achieved / peak_tf, "traffic": None,
+                "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md section 7)",
+                "algorithmic": f"{algorithmic}, x {executed} executed terms per call; time = the transfer call"}
+        extra = {"executed_terms_per_s": executed / t_step, "spectra_per_s": 1.0 / t_step}
+        stride = max(1, k.size // max(2 * cores, 16))          # a bounded k sample, every cost class represented
+        sl = slice(0, k.size, stride)
+        ref(sl)                                                # warm the oracle's threads
+        t0 = time.perf_counter()
+        D_ref = ref(sl)
+        dt = time.perf_counter() - t0
+        rows = np.arange(k.size)[sl]
+        D_gpu = get_rows(torch.from_numpy(rows).to(dev)).cpu().numpy()
+        scale = np.max(np.abs(D_ref), axis=-1, keepdims=True)
+        err = float(np.max(np.abs(D_gpu - D_ref) / np.where(scale > 0, scale, 1.0)))
+        cpu = {"value": units / k.size * rows.size / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"every {stride}-th k row ({rows.size} of {k.size}), fp64 oracle build, {dt:.1f} s",
+               "delta_err_on_sample": err}
+    out_line = {
+        "metric": metric, "value": value, "unit": unit, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": workload, "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB memset)"},
+        **{n: t for n, t in zip(names, times)}, **extra, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out_line), flush=True)
+    plan.close()
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -445,8 +621,16 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=1, choices=range(len(synth.CONFIGS)))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="config", choices=["config", "sparse", "tensor", "open", "srcinterp"],
+                    help="config: BASELINE.json's configs (--config); the others: SURVEY 8(f) rows, one GPU")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.workload != "config":
+        if args.impl != "cuda" or args.gpus != 1:
+            raise SystemExit("bench.py: --workload rows run on one GPU with the CUDA arm only")
+        args.steps = 50 if args.steps is None else args.steps
+        args.warmup = 5 if args.warmup is None else max(args.warmup, 3)
+        run_next(args)
+    elif args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup
         run_reference(args)

@@ -242,35 +242,47 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
                 for (int h = 0; h < 2; ++h)
 #pragma unroll
                     for (int nb = 0; nb < NB; ++nb) D[h][nb][0] = D[h][nb][1] = 0.0;
+                // a2 for one slot: eight steps of the recurrence; j_l, .., j_{l-7} of this lane's tau go to tile `b`
+                auto recur = [&](int j, int b) {   // j is a constant once the slot loop is unrolled
+                    const double ixj = my_ix[j * F_THREADS];
+                    const double e = tl0 * my_ixlo[j * F_THREADS];
+                    double *tile_w = jt + (size_t)b * V * JS + lane;
+#pragma unroll
+                    for (int s = 0; s < V; ++s) {
+                        const double tl = tl0 - 2.0 * s;
+                        const double c = fma(tl, ixj, e);        // correctly rounded (2l+1)/x
+                        tile_w[s * JS] = fb[j];
+                        const double fn = fma(c, fb[j], -fa[j]);
+                        fa[j] = fb[j];
+                        fb[j] = fn;
+                    }
+                };
+                // Software pipeline over the slots: the recurrence of slot j + 1 (a dependent chain of 16 FP64
+                // instructions, latency-bound on its own) is issued between the A-fragment loads and the 16 MMAs
+                // of slot j, which do not depend on it; two tiles suffice (the __syncwarp orders the writes of
+                // slot j + 1 behind the reads of slot j - 1).
+                recur(0, buf);
 #pragma unroll
                 for (int j = 0; j < T; ++j) {
                     if (j < na) {
-                        // a2: eight steps of the recurrence; j_l, .., j_{l-7} of this lane's tau go to the tile
-                        const double ixj = my_ix[j * F_THREADS];
-                        const double e = tl0 * my_ixlo[j * F_THREADS];
-                        double *tile_w = jt + (size_t)buf * V * JS + lane;
-#pragma unroll
-                        for (int s = 0; s < V; ++s) {
-                            const double tl = tl0 - 2.0 * s;
-                            const double c = fma(tl, ixj, e);        // correctly rounded (2l+1)/x
-                            tile_w[s * JS] = fb[j];
-                            const double fn = fma(c, fb[j], -fa[j]);
-                            fa[j] = fb[j];
-                            fb[j] = fn;
-                        }
                         __syncwarp();
                         // a3: A fragments (row = l-row fr, column = tau 8 mm + 2 fc + {0,1}) x B fragments
                         const double2 *tile_r = reinterpret_cast<const double2 *>(jt + (size_t)buf * V * JS + fr * JS + 2 * fc);
+                        double2 a[4];
+#pragma unroll
+                        for (int mm = 0; mm < 4; ++mm) a[mm] = tile_r[4 * mm];
+                        // unconditional (a slot that has not started carries zeros and yields zeros): no branch between
+                        // the chain and the MMAs, so that the scheduler may interleave them
+                        if (j + 1 < T) recur(j + 1 < T ? j + 1 : 0, buf ^ 1);
 #pragma unroll
                         for (int mm = 0; mm < 4; ++mm) {
-                            const double2 a = tile_r[4 * mm];
 #pragma unroll
                             for (int nb = 0; nb < NB; ++nb) {
-                                dmma(D[0][nb], a.x, Bf[j][2 * mm][nb]);
-                                dmma(D[1][nb], a.y, Bf[j][2 * mm + 1][nb]);
+                                dmma(D[0][nb], a[mm].x, Bf[j][2 * mm][nb]);
+                                dmma(D[1][nb], a[mm].y, Bf[j][2 * mm + 1][nb]);
                             }
                         }
-                        buf ^= 1;   // the next slot writes the other tile: two tiles suffice (see __syncwarp above)
+                        buf ^= 1;
                     }
                 }
                 // D fragment: row fr, columns 2 fc, 2 fc + 1 of block nb = (T, E) of cosmology 4 nb + fc
