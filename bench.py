@@ -590,9 +590,13 @@ def run_next(args) -> None:
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md section 7)",
                 "algorithmic": f"{algorithmic}, x {executed} executed terms per call; time = the transfer call"}
         extra = {"executed_terms_per_s": executed / t_step, "spectra_per_s": 1.0 / t_step}
-        stride = max(1, k.size // max(2 * cores, 16))          # a bounded k sample, every cost class represented
+        # a bounded k sample (about 10 s of oracle time), evenly strided so that every cost class is represented
+        stride = max(1, k.size // max(2 * cores, 16))
+        t0 = time.perf_counter()
+        ref(slice(0, k.size, stride))
+        per_row = (time.perf_counter() - t0) / len(range(0, k.size, stride))
+        stride = max(1, -(-k.size // max(2, min(k.size, int(10.0 / max(per_row, 1e-9))))))
         sl = slice(0, k.size, stride)
-        ref(sl)                                                # warm the oracle's threads
         t0 = time.perf_counter()
         D_ref = ref(sl)
         dt = time.perf_counter() - t0
