@@ -41,11 +41,15 @@ UNIT = "terms/s"
 # FP64 roofline denominator: 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE gcamb_los_transfer call (its plain launch plus
-# its small compensated-rows launch), from the committed ncu --set full capture
-# (profiles/r1_transfer_kernel_plain.txt, r1_transfer_kernel_compensated.txt); only config 1 was captured
-NCU_TRAFFIC_BYTES = {1: (155.694336e6 + 91.366656e6) + (3.065088e6 + 0.0)}
-
+# dram__bytes_read.sum + dram__bytes_write.sum of the transfer call of ONE step (config 3: the fused call), summed over
+# its launches, from the committed ncu --set full captures (profiles/r2_kernels.md)
+NCU_TRAFFIC_BYTES = {
+    0: 5.308e6,
+    1: (155.7e6 + 91.24e6) + 3.062e6,
+    2: (1.466e9 + 1.327e9) + (0.09813e9 + 0.04122e9),
+    3: (5.63e9 + 2.026e9) + (0.5682e9 + 0.006468e9),
+    4: (3.948e9 + 4.605e9) + (0.4554e9 + 0.7074e9),
+}
 
 def host_cores() -> int:
     try:
@@ -407,7 +411,7 @@ def run_cuda(args) -> None:
         "roofline": {
             "bound": "alu", "kernel": kernel_name, "achieved": achieved_tf, "peak": peak_tf,
             "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-            "traffic_unit": "bytes per transfer call (ncu dram read+write, profiles/r1_transfer_kernel_*.txt)",
+            "traffic_unit": "bytes per transfer call (ncu dram read+write of its launches, profiles/r2_kernels.md)",
             "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md); "
                            f"dfma probe measured {probe_tf:.2f} TFLOP/s, dmma (m8n8k4.f64) probe "
                            f"{probe_dmma_tf:.2f} TFLOP/s in this process",
