@@ -179,28 +179,34 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
     auto flush_group = [&](int m) {
         const int stage = m % RD;
         const int gcount = min(G, n_walk - m * G);
-        mbar_wait(bar_full + 8 * stage, (m / RD) & 1);
+        // this thread's (l, cosmology) and its three partial spectra: the loads (L2 round trips: the
+        // source view showed 8 % of the warp time waiting for them behind the ring sums) are issued
+        // before the wait on the ring so that they travel under it
+        int li = -1;
         if (f_on && f_gi < gcount) {
             const int l = p.l_max - (t_begin + m * G + f_gi) * V - f_r;
-            const int li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
-            if (li >= 0) {
-                const double2 *e = reinterpret_cast<const double2 *>(
-                    ring + ((size_t)(stage * G + f_gi) * W) * P + (f_r * BC + f_b) * 2);
-                double dT = 0.0, dE = 0.0;
+            li = l >= p.l_min ? (p.l_contig ? l - p.l_min : p.l_index[l]) : -1;
+        }
+        const size_t sp = (size_t)p.n_l * BC;
+        double *c = cpart + (size_t)(li >= 0 ? li : 0) * BC + f_b;
+        double c0 = 0.0, c1 = 0.0, c2 = 0.0, pf = 0.0;
+        if (li >= 0) { c0 = c[0]; c1 = c[sp]; c2 = c[2 * sp]; pf = p.pref[li]; }
+        mbar_wait(bar_full + 8 * stage, (m / RD) & 1);
+        if (li >= 0) {
+            const double2 *e = reinterpret_cast<const double2 *>(
+                ring + ((size_t)(stage * G + f_gi) * W) * P + (f_r * BC + f_b) * 2);
+            double dT = 0.0, dE = 0.0;
 #pragma unroll
-                for (int wv = 0; wv < W; ++wv) {
-                    const double2 v = e[(size_t)wv * (P / 2)];
-                    dT += v.x;
-                    dE += v.y;
-                }
-                dE *= p.pref[li];
-                const double wT = f_wk * dT, wE = f_wk * dE;
-                double *c = cpart + (size_t)li * BC + f_b;
-                const size_t sp = (size_t)p.n_l * BC;
-                c[0] = fma(wT, dT, c[0]);
-                c[sp] = fma(wE, dE, c[sp]);
-                c[2 * sp] = fma(wT, dE, c[2 * sp]);
+            for (int wv = 0; wv < W; ++wv) {
+                const double2 v = e[(size_t)wv * (P / 2)];
+                dT += v.x;
+                dE += v.y;
             }
+            dE *= pf;
+            const double wT = f_wk * dT, wE = f_wk * dE;
+            c[0] = fma(wT, dT, c0);
+            c[sp] = fma(wE, dE, c1);
+            c[2 * sp] = fma(wT, dE, c2);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8 * stage);
