@@ -62,6 +62,12 @@ def _lib(real: str) -> ctypes.CDLL:
             lib.oracle_cls_tensor.argtypes = [ctypes.c_int, _pd, ctypes.c_int, _pd, _pd, ctypes.c_int, _pd]
             lib.oracle_hyp_lcut_open.argtypes = [ctypes.c_double, ctypes.c_double]
             lib.oracle_hyp_lcut_open.restype = ctypes.c_int
+            lib.oracle_hyp_lcut_closed.argtypes = [ctypes.c_double, ctypes.c_double]
+            lib.oracle_hyp_lcut_closed.restype = ctypes.c_int
+            lib.oracle_hyp_bessel_closed.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, _pd]
+            lib.oracle_transfer_closed.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
+                                                   ctypes.c_double, ctypes.c_double, _pd, _pd, _pd, ctypes.c_int,
+                                                   ctypes.c_int, _pd]
             lib.oracle_hyp_bessel_open.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, _pd]
             lib.oracle_transfer_open.argtypes = [_pi, ctypes.c_int, _pd, ctypes.c_int, _pd, ctypes.c_int,
                                                  ctypes.c_double, ctypes.c_double, _pd, _pd, _pd, ctypes.c_int,
@@ -210,9 +216,21 @@ def hyp_bessel_open(beta: float, chi: float, lmax: int, margin: int = DEFAULT_MA
     return out
 
 
+def hyp_lcut_closed(beta: float, chi: float) -> int:
+    return _lib("f64").oracle_hyp_lcut_closed(float(beta), float(chi))
+
+
+def hyp_bessel_closed(beta: float, chi: float, lmax: int, margin: int = DEFAULT_MARGIN, real: str = "f64") -> np.ndarray:
+    """Hyperspherical Bessel functions of a closed universe (integer beta >= 3, chi <= pi/2), zero for l >= beta."""
+    out = np.empty(lmax + 1, dtype=np.float64)
+    if _lib(real).oracle_hyp_bessel_closed(float(beta), float(chi), int(lmax), int(margin), _ptr(out)):
+        raise ValueError("oracle_hyp_bessel_closed: bad arguments")
+    return out
+
+
 def transfer_open(l_list, k, tau, tau0, curv_K, S_T, S_E, S_phi=None, margin: int = DEFAULT_MARGIN,
                   real: str = "f64", nthreads: int = 0) -> np.ndarray:
-    """Delta[n_src][n_l][n_k] in an open universe of curvature curv_K < 0 (reading R28)."""
+    """Delta[n_src][n_l][n_k] in a curved universe: curv_K < 0 open, > 0 closed (reading R28)."""
     l_list = np.ascontiguousarray(l_list, dtype=np.int32)
     k, tau, S_T, S_E = _f64(k), _f64(tau), _f64(S_T), _f64(S_E)
     assert S_T.shape == (k.size, tau.size) and S_E.shape == S_T.shape
@@ -221,9 +239,13 @@ def transfer_open(l_list, k, tau, tau0, curv_K, S_T, S_E, S_phi=None, margin: in
         S_phi = _f64(S_phi)
         sp = _ptr(S_phi)
     out = np.empty((3 if S_phi is not None else 2, l_list.size, k.size), dtype=np.float64)
-    rc = _lib(real).oracle_transfer_open(l_list.ctypes.data_as(_pi), l_list.size, _ptr(k), k.size, _ptr(tau),
+    fn = _lib(real).oracle_transfer_open if curv_K < 0 else _lib(real).oracle_transfer_closed
+    rc = fn(l_list.ctypes.data_as(_pi), l_list.size, _ptr(k), k.size, _ptr(tau),
                                          tau.size, float(tau0), float(curv_K), _ptr(S_T), _ptr(S_E), sp,
                                          int(margin), int(nthreads), _ptr(out))
     if rc:
-        raise ValueError(f"oracle_transfer_open failed ({rc})")
+        raise ValueError(f"oracle_transfer_open/closed failed ({rc})")
     return out
+
+
+transfer_curved = transfer_open      # curv_K < 0: open, curv_K > 0: closed
