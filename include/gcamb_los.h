@@ -81,33 +81,36 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out,
                                    double tau0, uint32_t src_mask, void *cuda_stream);
 
 /*
- * Plan for an OPEN universe ("hyperspherical Bessel functions in a non-flat" Universe,
- * PAPER.md:60; DoNonFlatIntegration, the paper's "immediate next step").  The paper
- * gives no formula; reading R28: curvature K < 0 (in the units of k^2), r_c = 1/sqrt(-K),
- * beta_j = k_j r_c (the caller's k is the generalised wavenumber q = beta sqrt(-K)), chi_i = (tau0 -
- * tau_i)/r_c, and the radial functions are the hyperspherical Bessel functions Phi_l^beta(chi): the
- * regular solutions of  Phi'' + 2 coth(chi) Phi' + [beta^2 + 1 - l(l+1)/sinh^2(chi)] Phi = 0  with
- * Phi_0 = sin(beta chi)/(beta sinh chi), which obey
- *   sqrt(beta^2+(l+1)^2) Phi_{l+1} = (2l+1) coth(chi) Phi_l - sqrt(beta^2+l^2) Phi_{l-1}
- * and tend to j_l(beta chi) as K -> 0.  The transfer functions are the flat ones with j_l(x) ->
- * Phi_l^beta(chi) and, in the polarisation weight, x -> beta sinh(chi):
- *   Delta^T = sum w S_T Phi_l,  Delta^E = sqrt((l+2)!/(l-2)!) sum w S_E Phi_l/(beta sinh chi)^2,
+ * Plan for a CURVED universe ("hyperspherical Bessel functions in a non-flat" Universe,
+ * PAPER.md:60; DoNonFlatIntegration, the paper's "immediate next step").  The paper gives
+ * no formula; reading R28: curvature K != 0 (in the units of k^2), r_c = 1/sqrt|K|,
+ * beta_j = k_j r_c (the caller's k is the generalised wavenumber q = beta sqrt|K|), chi_i = (tau0 - tau_i)/r_c,
+ * and the radial functions are the hyperspherical Bessel functions Phi_l^beta(chi), the regular solutions of
+ *   K < 0 (open):   Phi'' + 2 coth(chi) Phi' + [beta^2 + 1 - l(l+1)/sinh^2(chi)] Phi = 0,  b_l = sqrt(beta^2 + l^2)
+ *   K > 0 (closed): Phi'' + 2 cot(chi)  Phi' + [beta^2 - 1 - l(l+1)/sin^2(chi)]  Phi = 0,  b_l = sqrt(beta^2 - l^2)
+ * with Phi_0 = sin(beta chi)/(beta sinK chi) (sinK = sinh or sin), which obey
+ *   b_{l+1} Phi_{l+1} = (2l+1) cotK(chi) Phi_l - b_l Phi_{l-1}
+ * and tend to j_l(beta chi) as K -> 0.  The transfer functions are the flat ones with j_l(x) -> Phi_l^beta(chi)
+ * and, in the polarisation weight, x -> beta sinK(chi):
+ *   Delta^T = sum w S_T Phi_l,  Delta^E = sqrt((l+2)!/(l-2)!) sum w S_E Phi_l/(beta sinK chi)^2,
  *   Delta^phi = sum w S_phi Phi_l;  Eq. 1 is taken over unchanged (the curved-space measure and spectrum
- * belong to the P the caller passes).  Skip rule (R16 in curved space): Phi_l := 0 above the first l at
- * which the product of the per-l decay ratios above the turning point l + 1/2 = beta sinh(chi) has fallen
- * below 1e-36 (those ratios tend to tanh(chi/2): slower than the flat j_l when chi is not small).
- * The plan holds, next to the tables of gcamb_los_plan_create, coth(chi_i) and 1/sinh^2(chi_i) per tau and
+ * belong to the P the caller passes).  Skip rule (R16 in curved space): Phi_l := 0 above the first l at which the
+ * product of the per-l decay ratios above the turning point l + 1/2 = beta sinK(chi) has fallen below 1e-36
+ * (open: those ratios tend to tanh(chi/2), slower than the flat j_l when chi is not small).
+ * Closed universes: every beta_j must be an integer >= 3 (to 1e-6; it is rounded to it) and chi <= pi/2 on the
+ * whole tau grid (GCAMB_EGRID otherwise); Phi_l^beta = 0, hence Delta_l(k_j) = 0 exactly, for l >= beta_j.
+ * The plan holds, next to the tables of gcamb_los_plan_create, cotK(chi_i) and 1/sinK^2(chi_i) per tau and
  * the two recurrence coefficients per (k, l): 16 n_l n_k bytes.  gcamb_los_transfer[_batched],
  * gcamb_los_cls[_batched], gcamb_los_spectra_host, gcamb_los_cl_interp and gcamb_los_srcinterp_create work
- * on such a plan as on a flat one (gcamb_los_spectra_batched takes its two-kernel path).  K > 0 (closed
- * universes: integer beta, l < beta) is not built: GCAMB_EINVAL.  src_mask: T|E or T|E|PHI.
+ * on such a plan as on a flat one (gcamb_los_spectra_batched takes its two-kernel path).
+ * src_mask: T|E or T|E|PHI.  K = 0 is GCAMB_EINVAL (use gcamb_los_plan_create).
  */
-gcamb_status gcamb_los_plan_create_open(gcamb_los_plan **out,
-                                        const int32_t *l_list, int32_t n_l,
-                                        const double *k, int32_t n_k,
-                                        const double *tau, int32_t n_tau,
-                                        double tau0, double curvature_K, uint32_t src_mask,
-                                        void *cuda_stream);
+gcamb_status gcamb_los_plan_create_curved(gcamb_los_plan **out,
+                                          const int32_t *l_list, int32_t n_l,
+                                          const double *k, int32_t n_k,
+                                          const double *tau, int32_t n_tau,
+                                          double tau0, double curvature_K, uint32_t src_mask,
+                                          void *cuda_stream);
 
 /* Frees the plan and its device tables (synchronises the device).  NULL is allowed. */
 gcamb_status gcamb_los_plan_destroy(gcamb_los_plan *plan);

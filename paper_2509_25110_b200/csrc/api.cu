@@ -56,7 +56,7 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
     cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg); cudaFree(p->d_l_user);
-    cudaFree(p->d_cth); cudaFree(p->d_s2); cudaFree(p->d_ib2); cudaFree(p->d_coef);
+    cudaFree(p->d_cth); cudaFree(p->d_s2); cudaFree(p->d_ib2); cudaFree(p->d_coef); cudaFree(p->d_l_end);
     cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_cE); cudaFree(p->d_t_cB);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
@@ -117,10 +117,8 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     if (!out || !l_list || !k || !tau) { set_error("null argument"); return GCAMB_EINVAL; }
     if (n_l < 1 || n_k < 2 || n_tau < 2) { set_error("need n_l >= 1, n_k >= 2, n_tau >= 2"); return GCAMB_EINVAL; }
     const bool curved = curv_K != 0.0;
-    if (curved && !(curv_K < 0.0 && std::isfinite(curv_K))) {
-        set_error("curvature K must be negative and finite: closed universes (integer beta) are not built");
-        return GCAMB_EINVAL;
-    }
+    if (!std::isfinite(curv_K)) { set_error("curvature K must be finite"); return GCAMB_EINVAL; }
+    const int sgn = curv_K < 0.0 ? +1 : -1;     // +1 open, -1 closed
     const bool tensor = src_mask == GCAMB_SRC_TENSOR;
     if (curved && tensor) { set_error("tensor plans are flat only"); return GCAMB_EINVAL; }
     if (!tensor && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E) && src_mask != (GCAMB_SRC_T | GCAMB_SRC_E | GCAMB_SRC_PHI)) {
@@ -163,8 +161,8 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     p->n_l = n_l; p->n_k = n_k; p->n_tau = n_tau;
     p->n_l_out = n_user;
     p->tensor = tensor;
-    p->curved = curved;
-    p->r_c = curved ? 1.0 / std::sqrt(-curv_K) : 0.0;
+    p->curved = curved ? sgn : 0;
+    p->r_c = curved ? 1.0 / std::sqrt(std::fabs(curv_K)) : 0.0;
     p->src_mask = src_mask;
     p->n_src = (tensor || (src_mask & GCAMB_SRC_PHI)) ? 3 : 2;
     p->n_spec = p->n_src + 1;
@@ -184,16 +182,33 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     std::vector<double> vk(k, k + n_k), vtau(tau, tau + n_tau), chi(n_tau), lnk(n_k), pref(n_l);
     for (int i = 0; i < n_tau; ++i) chi[i] = tau0 - tau[i];
     std::vector<double> cth, s2, ib2;
-    if (curved) {   // chi_i = sqrt(-K) (tau0 - tau_i), one rounding, like the flat x = k chi; beta_j = k_j r_c
-        const double sk = std::sqrt(-curv_K);
+    if (curved) {   // chi_i = sqrt|K| (tau0 - tau_i), one rounding, like the flat x = k chi; beta_j = k_j r_c
+        const double sk = std::sqrt(std::fabs(curv_K));
         cth.resize(n_tau); s2.resize(n_tau); ib2.resize(n_k);
         for (int i = 0; i < n_tau; ++i) {
             chi[i] = sk * (tau0 - tau[i]);
-            const double sh = std::sinh(chi[i]);
-            cth[i] = std::cosh(chi[i]) / sh;
+            const double sh = sgn > 0 ? std::sinh(chi[i]) : std::sin(chi[i]);
+            cth[i] = (sgn > 0 ? std::cosh(chi[i]) : std::cos(chi[i])) / sh;
             s2[i] = 1.0 / (sh * sh);
         }
-        for (int j = 0; j < n_k; ++j) { const double beta = k[j] * p->r_c; ib2[j] = 1.0 / (beta * beta); }
+        if (sgn < 0 && !(chi[0] <= 1.5707963267948966)) {
+            set_error("closed universe: chi = sqrt(K) (tau0 - tau) must not exceed pi/2 (it is %.4f at tau[0])", chi[0]);
+            free_plan(p);
+            return GCAMB_EGRID;
+        }
+        for (int j = 0; j < n_k; ++j) {
+            double beta = k[j] * p->r_c;
+            if (sgn < 0) {   // closed: the modes are beta = 3, 4, 5, ...
+                const double br = std::floor(beta + 0.5);
+                if (br < 3.0 || std::fabs(beta - br) > 1e-6 * br) {
+                    set_error("closed universe: k[%d] / sqrt(K) = %.9g is not an integer >= 3", j, beta);
+                    free_plan(p);
+                    return GCAMB_EGRID;
+                }
+                beta = br;
+            }
+            ib2[j] = 1.0 / (beta * beta);
+        }
     }
     for (int j = 0; j < n_k; ++j) lnk[j] = std::log(k[j]);
     std::vector<double> w = trapezoid(vtau), dlnk = trapezoid(lnk);
@@ -244,6 +259,7 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
         if (e == cudaSuccess) e = upload(&p->d_s2, s2, stream);
         if (e == cudaSuccess) e = upload(&p->d_ib2, ib2, stream);
         if (e == cudaSuccess) e = cudaMalloc(&p->d_coef, sizeof(double2) * (size_t)n_k * p->n_tiles * p->shape.V);
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_l_end, sizeof(int32_t) * n_k);
     }
     if (e == cudaSuccess) e = cudaMalloc(&p->d_korder, sizeof(int32_t) * n_k);
     // the uploads read pageable vectors that die with this scope
@@ -266,13 +282,13 @@ gcamb_status gcamb_los_plan_create(gcamb_los_plan **out, const int32_t *l_list, 
     return create_plan(out, l_list, n_l, k, n_k, tau, n_tau, tau0, 0.0, src_mask, cuda_stream);
 }
 
-gcamb_status gcamb_los_plan_create_open(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
-                                        const double *k, int32_t n_k, const double *tau, int32_t n_tau,
-                                        double tau0, double curvature_K, uint32_t src_mask, void *cuda_stream)
+gcamb_status gcamb_los_plan_create_curved(gcamb_los_plan **out, const int32_t *l_list, int32_t n_l,
+                                          const double *k, int32_t n_k, const double *tau, int32_t n_tau,
+                                          double tau0, double curvature_K, uint32_t src_mask, void *cuda_stream)
 {
-    if (!(curvature_K < 0.0)) {
+    if (!(curvature_K != 0.0)) {
         if (out) *out = nullptr;
-        set_error("gcamb_los_plan_create_open needs K < 0 (K = 0: gcamb_los_plan_create; K > 0 is not built)");
+        set_error("gcamb_los_plan_create_curved needs K != 0 (K = 0: gcamb_los_plan_create)");
         return GCAMB_EINVAL;
     }
     return create_plan(out, l_list, n_l, k, n_k, tau, n_tau, tau0, curvature_K, src_mask, cuda_stream);

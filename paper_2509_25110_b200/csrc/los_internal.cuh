@@ -24,7 +24,7 @@ struct gcamb_los_plan {
     int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
     int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l and l + 1)
     int32_t tensor;          // tensor-mode plan (tensor.cu)
-    int32_t curved;          // open-universe plan (reading R28): hyperspherical Bessel functions
+    int32_t curved;          // 0 flat; +1 open, -1 closed universe (reading R28): hyperspherical Bessel functions
     double r_c;              // curvature radius 1/sqrt(-K) (curved plans)
     uint32_t src_mask;
     double tau0;
@@ -73,6 +73,7 @@ struct gcamb_los_plan {
     double *d_s2;            // [n_tau] 1/sinh^2(chi_i)
     double *d_ib2;           // [n_k]   1/beta_j^2, beta_j = k_j r_c
     double2 *d_coef;         // [n_k][n_tiles V] (A_l, R_l) = ((2l+1)/b_l, b_{l+1}/b_l), l = l_max - index
+    int32_t *d_l_end;        // [n_k]   closed: beta - 1, the last l with a non-zero function; open: INT_MAX
 
     // tensor plans: positions of l and l + 1 of the caller's list in l_list, combination coefficients
     int32_t *d_t_pos0, *d_t_pos1;   // [n_l_out]

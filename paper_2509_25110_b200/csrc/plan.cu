@@ -43,26 +43,35 @@ __device__ __forceinline__ double j1_series(double x)
 // Above the turning point l + 1/2 = beta sinh(chi) the regular solution falls by the smaller root r_l of
 // b_{l+1} r^2 - (2l+1) coth(chi) r + b_l = 0 per step (-> tanh(chi/2) for l >> beta, slower than the flat
 // j_l when chi is not small): the cut is the first l at which the product of the r_l is below 1e-36, + 8.
-__device__ __forceinline__ int l_cut_open(double beta, double cth, double x_turn)
+// sgn = +1: open (b_l^2 = beta^2 + l^2); sgn = -1: closed (b_l^2 = beta^2 - l^2, integer beta, Phi_l = 0 for
+// l >= beta: the cut never exceeds beta - 1, the end of the ladder).
+__device__ __forceinline__ double b_curved(double b2, int l, int sgn)
+{
+    const double v = fma((double)(sgn * l), (double)l, b2);
+    return v > 0.0 ? sqrt(v) : 0.0;
+}
+
+__device__ __forceinline__ int l_cut_curved(double beta, double cth, double x_turn, int sgn)
 {
     int l = max(1, (int)ceil(x_turn));
+    const int top = sgn > 0 ? 4000000 : (int)beta - 1;
     double lg = 0.0;
     const double b2 = beta * beta;
-    while (lg > -82.9 && l < 4000000) {
-        const double bl = sqrt(fma((double)l, (double)l, b2)), bl1 = sqrt(fma((double)(l + 1), (double)(l + 1), b2));
+    while (lg > -82.9 && l < top) {
+        const double bl = b_curved(b2, l, sgn), bl1 = b_curved(b2, l + 1, sgn);
         const double t = (double)(2 * l + 1) * cth;
         const double disc = fma(t, t, -4.0 * bl * bl1);
         if (disc > 0.0) lg += log(2.0 * bl / (t + sqrt(disc)));
         ++l;
     }
-    return l + 8;
+    return min(l + 8, top);
 }
 
 // CURVED: `chi` holds chi_i = (tau0 - tau_i)/r_c and `k` is multiplied by r_c to give beta; inv_x is not written.
 template <bool CURVED>
 __global__ void __launch_bounds__(128) start_values_kernel(const double *__restrict__ k,
                                                            const double *__restrict__ chi, int n_tau,
-                                                           int l_max, int V, double r_c,
+                                                           int l_max, int V, double r_c, int sgn,
                                                            double2 *__restrict__ start,
                                                            int32_t *__restrict__ tile,
                                                            double *__restrict__ inv_x,
@@ -71,27 +80,34 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
     const int i = blockIdx.y * blockDim.x + threadIdx.x;   // k along grid.x: n_k is bounded by 2^31 - 1 only
     const int j = blockIdx.x;
     if (i >= n_tau) return;
-    const double beta = CURVED ? __dmul_rn(k[j], r_c) : 0.0;
+    double beta = CURVED ? __dmul_rn(k[j], r_c) : 0.0;
+    if (CURVED && sgn < 0) beta = rint(beta);          // closed: integer beta (validated at plan creation)
     const double ch = chi[i];
     const double x = CURVED ? __dmul_rn(beta, ch) : __dmul_rn(k[j], ch);
-    const double snh = CURVED ? sinh(ch) : 0.0, cth = CURVED ? cosh(ch) / snh : 0.0;
-    const int L = CURVED ? l_cut_open(beta, cth, beta * snh) : l_cut(x);
+    const double snh = CURVED ? (sgn > 0 ? sinh(ch) : sin(ch)) : 0.0;
+    const double cth = CURVED ? (sgn > 0 ? cosh(ch) : cos(ch)) / snh : 0.0;
+    const int L = CURVED ? l_cut_curved(beta, cth, beta * snh, sgn) : l_cut(x);
     const int Ls = min(L, l_max);
     const int t = (l_max - Ls) / V;
     const int lhi = l_max - t * V;  // Ls <= lhi < Ls + V
-    const int M = max(L, lhi) + 50;
+    // closed: the ladder ends at top = beta - 1 (b_beta = 0).  When the start tile reaches above it, the levels
+    // l >= beta are walked with the coefficients (0, -1) of curved_coef_kernel, which keep a constant sequence:
+    // the pair handed to the transfer kernel is then (Phi_top, Phi_top), and the flush zeroes Delta_l for l > top.
+    const int top = (CURVED && sgn < 0) ? (int)beta - 1 : 0x7fffffff;
+    const int M = min(max(L, lhi) + 50, top);
+    const int l_cap = min(lhi, top);       // level at which the pair is taken
     if (CURVED) cut[(size_t)j * n_tau + i] = Ls;
 
     double fa = 0.0, fb = 1.0;  // f_{l+1}, f_l
     double rhi = 0.0, rlo = 0.0;
     int e = 0, re = 0;
     const double b2 = beta * beta;
-    double b_up = CURVED ? sqrt(fma((double)(M + 1), (double)(M + 1), b2)) : 0.0;   // b_{l+1}
+    double b_up = CURVED ? b_curved(b2, M + 1, sgn) : 0.0;   // b_{l+1}
     for (int l = M; l >= 1; --l) {
-        if (l == lhi) { rlo = fb; rhi = fa; re = e; }
+        if (l == l_cap) { rlo = fb; rhi = (lhi > top) ? fb : fa; re = e; }
         double fn;
         if (CURVED) {
-            const double bl = sqrt(fma((double)l, (double)l, b2));
+            const double bl = b_curved(b2, l, sgn);
             fn = ((double)(2 * l + 1) * cth * fb - b_up * fa) / bl;
             b_up = bl;
         } else {
@@ -112,7 +128,7 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
         // closed form of Phi_1 cancels and Phi_0 ~ 1 alone fixes the scale
         const double d = 1.0 / (beta * snh);
         j0 = s * d;
-        j1 = x < 1.0 ? fa * (j0 / fb) : (cth * s - beta * c) * d / sqrt(b2 + 1.0);
+        j1 = x < 1.0 ? fa * (j0 / fb) : (cth * s - beta * c) * d / b_curved(b2, 1, sgn);
     } else {
         j0 = s * inv;
         j1 = x < 1.0 ? j1_series(x) : (s * inv - c) * inv;
@@ -136,16 +152,23 @@ __global__ void __launch_bounds__(128) start_values_kernel(const double *__restr
 
 // Open universe: per (k, l) the two coefficients of a downward step  Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1},
 // A_l = (2l+1)/b_l, R_l = b_{l+1}/b_l, laid out as the transfer kernel walks: [k][tile][step], l = l_max - tile V - step
-__global__ void __launch_bounds__(256) curved_coef_kernel(const double *__restrict__ k, double r_c, int l_max, int n_walk,
-                                                          double2 *__restrict__ coef)
+// Closed universes: (0, -1) for l >= beta (see start_values_kernel), R_{beta-1} = b_beta / b_{beta-1} = 0 by itself;
+// l_end[k] = beta - 1, the last multipole with a non-zero function (open: none).
+__global__ void __launch_bounds__(256) curved_coef_kernel(const double *__restrict__ k, double r_c, int sgn, int l_max, int n_walk,
+                                                          double2 *__restrict__ coef, int32_t *__restrict__ l_end)
 {
     const int j = blockIdx.y;
-    const double beta = __dmul_rn(k[j], r_c), b2 = beta * beta;
+    double beta = __dmul_rn(k[j], r_c);
+    if (sgn < 0) beta = rint(beta);
+    const double b2 = beta * beta;
+    if (blockIdx.x == 0 && threadIdx.x == 0) l_end[j] = sgn < 0 ? (int)beta - 1 : 0x7fffffff;
     for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < n_walk; a += gridDim.x * blockDim.x) {
         const int l = l_max - a;
         double2 c = make_double2(0.0, 0.0);
-        if (l >= 1) {
-            const double bl = sqrt(fma((double)l, (double)l, b2)), bl1 = sqrt(fma((double)(l + 1), (double)(l + 1), b2));
+        if (sgn < 0 && (double)l >= beta) {
+            c = make_double2(0.0, -1.0);
+        } else if (l >= 1) {
+            const double bl = b_curved(b2, l, sgn), bl1 = b_curved(b2, l + 1, sgn);
             c = make_double2((double)(2 * l + 1) / bl, bl1 / bl);
         }
         coef[(size_t)j * n_walk + a] = c;
@@ -191,18 +214,18 @@ gcamb_status plan_precompute(gcamb_los_plan *p, cudaStream_t stream)
     int32_t *d_cut = nullptr;
     if (p->curved) {
         GCAMB_CUDA(cudaMalloc(&d_cut, sizeof(int32_t) * (size_t)p->n_k * p->n_tau));
-        start_values_kernel<true><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, p->r_c,
+        start_values_kernel<true><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, p->r_c, p->curved,
                                                             p->d_start, p->d_tile, nullptr, d_cut);
         cudaError_t ec = cudaGetLastError();
         if (ec == cudaSuccess) {
             const int n_walk = p->n_tiles * V;
             curved_coef_kernel<<<dim3((unsigned)((n_walk + 255) / 256), (unsigned)p->n_k), 256, 0, stream>>>(
-                p->d_k, p->r_c, p->l_max, n_walk, p->d_coef);
+                p->d_k, p->r_c, p->curved, p->l_max, n_walk, p->d_coef, p->d_l_end);
             ec = cudaGetLastError();
         }
         if (ec != cudaSuccess) { cudaFree(d_cut); return cuda_fail(ec, "plan precompute (open universe)"); }
     } else {
-        start_values_kernel<false><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, 0.0,
+        start_values_kernel<false><<<grid, 128, 0, stream>>>(p->d_k, p->d_chi, p->n_tau, p->l_max, V, 0.0, 0,
                                                              p->d_start, p->d_tile, p->d_inv, nullptr);
         GCAMB_CUDA(cudaGetLastError());
     }

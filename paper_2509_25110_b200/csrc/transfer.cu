@@ -58,6 +58,7 @@ struct TransferParams {
     // open-universe plans (CURVED kernels, reading R28); appended so that the flat kernels see the same layout
     const double *cth, *s2, *ib2;   // coth(chi_i), 1/sinh^2(chi_i) [n_tau]; 1/beta_j^2 [n_k]
     const double2 *coef;            // [n_k][n_tiles V] (A_l, R_l) of the step Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1}
+    const int32_t *l_end;           // [n_k] closed universes: Delta_l(k) = 0 for l > l_end[k] = beta_k - 1 (open: INT_MAX)
 };
 
 constexpr int T_MAX = 12;      // points per thread: the NA dispatch of the kernel is written out up to 12
@@ -223,6 +224,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
     // the cost order is the k grid reversed whenever cost grows with k: no table look-up then
     const int kidx = p.order_reversed ? p.n_k - 1 - krank : __reduce_min_sync(0xffffffffu, p.korder[krank]);   // uniform register, like the bookkeeping below
     const double kval = p.k[kidx];
+    const int l_end = CURVED ? p.l_end[kidx] : 0x7fffffff;
     const size_t row = (size_t)kidx * p.n_tau;
     const size_t delta_b = (size_t)b * NSRC * p.n_l;
 #define DIDX(q, li) (delta_b + (size_t)(q) * p.n_l + (li)) * p.n_k + kidx
@@ -334,6 +336,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             if (idx < G * P && l >= p.l_min) li = p.l_contig ? l - p.l_min : p.l_index[l];
             f_li[o] = li;
             f_pref[o] = (q == 1 && li >= 0) ? p.pref[li] : 1.0;
+            if (CURVED && l > l_end) f_pref[o] = 0.0;   // closed universe: no function above beta - 1 (the walk carries a constant there)
         }
     };
 
@@ -370,6 +373,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                     double sum = 0.0;
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * WM + wv) * P + r];
                     if (q == 1) sum *= p.pref[li];
+                    if (CURVED && l > l_end) sum = 0.0;
                     double *dst = p.Delta + DIDX(q, li);
                     *dst = (MULTI && pass) ? *dst + sum : sum;
                 }
@@ -693,7 +697,7 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.n_batch = n_batch; prm.n_pass = sh.n_pass; prm.pass_len = sh.pass_len;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
     prm.order_reversed = p->order_reversed;
-    prm.cth = p->d_cth; prm.s2 = p->d_s2; prm.ib2 = p->d_ib2; prm.coef = p->d_coef;
+    prm.cth = p->d_cth; prm.s2 = p->d_s2; prm.ib2 = p->d_ib2; prm.coef = p->d_coef; prm.l_end = p->d_l_end;
     if (p->curved)
         return (p->n_src == 2 ? launch_range_curved_2 : launch_range_curved_3)(prm, sh, 0, pos0, pos1, zero_fill, p->device, stream);
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l

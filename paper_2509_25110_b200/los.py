@@ -19,7 +19,7 @@ GCAMB_SRC_T, GCAMB_SRC_E, GCAMB_SRC_PHI, GCAMB_SRC_TENSOR = 1, 2, 4, 8
 _STATUS = {0: "GCAMB_OK", 1: "GCAMB_EINVAL", 2: "GCAMB_EGRID", 3: "GCAMB_EALLOC", 4: "GCAMB_ECUDA"}
 
 EXPORTS = (
-    "gcamb_los_plan_create", "gcamb_los_plan_create_open", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
+    "gcamb_los_plan_create", "gcamb_los_plan_create_curved", "gcamb_los_plan_destroy", "gcamb_los_plan_info", "gcamb_los_plan_launches",
     "gcamb_los_transfer",
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
     "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
@@ -52,7 +52,7 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_last_error.restype = ctypes.c_char_p
     lib.gcamb_los_plan_create.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64,
                                           ctypes.c_uint32, _vp]
-    lib.gcamb_los_plan_create_open.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64, _f64,
+    lib.gcamb_los_plan_create_curved.argtypes = [ctypes.POINTER(_vp), _vp, _i32, _vp, _i32, _vp, _i32, _f64, _f64,
                                                ctypes.c_uint32, _vp]
     lib.gcamb_los_plan_destroy.argtypes = [_vp]
     lib.gcamb_los_plan_info.argtypes = [_vp] + [ctypes.POINTER(_i32)] * 5 + [ctypes.POINTER(_i64)]
@@ -121,8 +121,8 @@ class Plan:
         mask = GCAMB_SRC_TENSOR if tensor else GCAMB_SRC_T | GCAMB_SRC_E | (GCAMB_SRC_PHI if with_phi else 0)
         self.tensor = bool(tensor)
         handle = _vp()
-        if curvature_K != 0.0:      # open universe (K < 0); the library rejects K > 0
-            _check(lib.gcamb_los_plan_create_open(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
+        if curvature_K != 0.0:      # K < 0 open, K > 0 closed universe
+            _check(lib.gcamb_los_plan_create_curved(ctypes.byref(handle), l_list.ctypes.data, l_list.size,
                                                   k.ctypes.data, k.size, tau.ctypes.data, tau.size,
                                                   float(tau0), float(curvature_K), mask, _stream()))
         else:

@@ -1,5 +1,5 @@
-"""SURVEY 8(f) NEXT-4 on the GPU: line-of-sight integration in an OPEN universe (hyperspherical Bessel
-functions, reading R28), element by element against the long-double oracle
+"""SURVEY 8(f) NEXT-4 on the GPU: line-of-sight integration in OPEN and CLOSED universes (hyperspherical
+Bessel functions, reading R28), element by element against the long-double oracle
 (pinned in tests/test_oracle_curved.py).
 
 Bars as for the flat path: |dDelta| <= 1e-10 max_k|Delta_l| per (source, l); C_l 1e-8 (R13).
@@ -137,13 +137,85 @@ def test_open_universe_at_config1_tau_grid(los):
     plan.close()
 
 
-def test_closed_universes_and_tensor_curved_plans_are_rejected(los):
-    k = synth.k_grid(8, 1e-3, 0.01)
+def closed_k_grid(n_k, beta_lo, beta_hi, r_c):
+    """k = beta / r_c on n_k distinct integers beta, roughly log-spaced between beta_lo and beta_hi."""
+    beta = np.unique(np.rint(np.geomspace(beta_lo, beta_hi, 3 * n_k)).astype(np.int64))
+    beta = beta[np.linspace(0, beta.size - 1, n_k).astype(int)]
+    return beta, beta / r_c
+
+
+def closed_sources(cfg, k):
+    """BASELINE.json's source model evaluated on the quantised k grid of a closed universe (seeded noise)."""
+    tau = cfg.tau()[None, :]
+    kk = k[:, None]
+    g = np.exp(-((tau - 280.0) ** 2) / (2.0 * 20.0 ** 2)) / (20.0 * np.sqrt(2.0 * np.pi))
+    damp = np.exp(-((kk / 0.1) ** 2))
+    S_T = g * np.cos(kk * tau / np.sqrt(3.0)) * damp + 2.0 * np.exp(-(((tau - 11000.0) / 2000.0) ** 2)) * np.exp(-kk / 0.01)
+    S_E = g * kk * np.sin(kk * tau / np.sqrt(3.0)) * damp
+    S_P = np.exp(-(((tau - 9000.0) / 3000.0) ** 2)) * kk ** -2.0 * np.exp(-kk / 0.2) * np.ones_like(S_T)
+    out = []
+    for q, S in enumerate((S_T, S_E, S_P)):
+        u = synth.uniform_pm1(cfg.seed, 700 + q, 0, S.size).reshape(S.shape)
+        out.append(np.ascontiguousarray(S * (1.0 + 1e-3 * u)))
+    return out
+
+
+@pytest.mark.parametrize("case", [
+    # (l_max, n_k, beta_lo, beta_hi, n_tau_uniform, n_tau_log, with_phi, r_c): r_c >= 2 tau0/pi keeps chi <= pi/2
+    (200, 50, 3, 400, 120, 60, False, 12000.0),        # many rows end below l_max: Delta_l = 0 for l >= beta
+    (300, 40, 3, 2500, 200, 100, True, 9000.0),        # chi up to 1.54
+    (120, 30, 100, 6000, 90, 43, True, 30000.0),       # every row starts at the top tile
+    (90, 12, 3, 60, 1900, 1700, False, 15000.0),       # several tau passes; beta - 1 below l_max on every row
+    (200, 25, 50, 40000, 120, 60, False, 2.0e6),       # nearly flat
+])
+def test_closed_universe_against_the_oracle(los, case):
+    l_max, n_k, b_lo, b_hi, n_u, n_log, with_phi, r_c = case
+    cfg = synth.Config(9, "closed", 2, l_max, n_k, 1e-4, 0.1, n_u, n_log, with_phi)
+    K = 1.0 / r_c ** 2
+    beta, k = closed_k_grid(n_k, b_lo, b_hi, r_c)
+    tau = cfg.tau()
+    S_T, S_E, S_P = closed_sources(cfg, k)
+    if not with_phi:
+        S_P = None
+    P = 2.1e-9 * (k / 0.05) ** -0.035
+    plan = los.Plan(cfg.l_list(), k, tau, cfg.tau0, with_phi=with_phi, curvature_K=K)
+    D = torch.full((plan.n_src, plan.n_l, plan.n_k), float("nan"), dtype=torch.float64, device="cuda")
+    d_S = (dev(S_T), dev(S_E), None if S_P is None else dev(S_P))
+    plan.gcamb_los_transfer(*d_S, out=D)
+    C = plan.gcamb_los_cls(D, dev(P))
+    torch.cuda.synchronize()
+    assert torch.equal(D, plan.gcamb_los_transfer(*d_S))
+    D, C = D.cpu().numpy(), C.cpu().numpy()
+    assert np.all(np.isfinite(D)) and np.all(np.isfinite(C))
+    D_ref = oracle.transfer_curved(cfg.l_list(), k, tau, cfg.tau0, K, S_T, S_E, S_P, real="f80")
+    e = delta_err(D, D_ref)
+    assert np.all(e <= TOL_DELTA), (float(e.max()), np.unravel_index(np.argmax(e), e.shape))
+    # Phi_l^beta = 0 for l >= beta: exact zeros, on both sides
+    above = cfg.l_list()[None, :, None] >= beta[None, None, :]
+    assert np.all(D[np.broadcast_to(above, D.shape)] == 0.0) and np.all(D_ref[np.broadcast_to(above, D.shape)] == 0.0)
+    C_ref = oracle.cls(k, D_ref, P, real="f80")
+    live = cfg.l_list() < beta.max()              # above the largest beta every transfer function, hence C_l, is 0
+    assert np.all(C[:, ~live] == 0.0) and np.all(C_ref[:, ~live] == 0.0)
+    e_auto, e_te = cl_err(C[:, live], C_ref[:, live])
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
+def test_curved_plans_that_are_rejected(los):
     tau = np.linspace(100.0, 13000.0, 10)
     l_list = np.arange(2, 6, dtype=np.int32)
+    r_c = 10000.0
+    k_int = np.array([3.0, 4.0, 7.0, 12.0]) / r_c
+    los.Plan(l_list, k_int, tau, 14000.0, curvature_K=1.0 / r_c ** 2).close()          # a valid closed plan
     with pytest.raises(los.GcambError) as e:
-        los.Plan(l_list, k, tau, 14000.0, curvature_K=+1e-8)
-    assert e.value.status == 1 and "K < 0" in str(e.value)
+        los.Plan(l_list, np.array([3.0, 4.5, 7.0]) / r_c, tau, 14000.0, curvature_K=1.0 / r_c ** 2)
+    assert e.value.status == 2 and "integer" in str(e.value)
     with pytest.raises(los.GcambError) as e:
-        los.Plan(l_list, k, tau, 14000.0, tensor=True, curvature_K=-1e-8)
+        los.Plan(l_list, np.array([2.0, 4.0]) / r_c, tau, 14000.0, curvature_K=1.0 / r_c ** 2)        # beta < 3
+    assert e.value.status == 2
+    with pytest.raises(los.GcambError) as e:
+        los.Plan(l_list, k_int * (r_c / 5000.0), tau, 14000.0, curvature_K=1.0 / 5000.0 ** 2)        # chi up to 2.8 > pi/2
+    assert e.value.status == 2 and "pi/2" in str(e.value)
+    with pytest.raises(los.GcambError) as e:
+        los.Plan(l_list, k_int, tau, 14000.0, tensor=True, curvature_K=-1e-8)
     assert e.value.status == 1
