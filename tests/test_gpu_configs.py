@@ -16,16 +16,15 @@ Outputs are pre-filled with NaN so an element the kernels fail to write cannot p
 Bars as in test_gpu_parity.py: |dDelta| <= 1e-10 max_k|Delta_l| per (source, l); C_l 1e-8 (R13).
 
 Config 4, l > ~8500, sources T and E (reading R14): there the synthetic
-recombination signal is damped to 1e-26 ... 1e-32 and the tau-sum cancels down to the +-1e-3 noise,
-so that ANY fp64 evaluation sits at about 1e-10 of max_k|Delta_l|: the fp64 build of the oracle
-itself differs from the long-double build by up to 1.2e-10 there.  The tolerance is not loosened
-silently: an l may exceed 1e-10 only where the fp64 oracle comes within a factor 2 of the same error
-(largest fp64-oracle error within 512 l: the errors are noise-like from one l to the next), the
-largest GPU error may not exceed 1.5 x the largest fp64-oracle error, and fewer than 1 % of the
-l may be over 1e-10.  The fp64 oracle is run on every k row as well, so both error profiles are
-maxima over the same 20000 rows.  DESIGN.md 6.3 carries the measured counts, and those of the one
-variant tried against it (coefficient carried as hi + lo through the recurrence step: more l over
-the bar, not fewer, at +21 % time).
+recombination signal is damped to 1e-26 ... 1e-32 and the tau-sum cancels down to the +-1e-3 noise, so
+that ANY fp64 evaluation loses five digits: over all 20000 k rows the fp64 build of the oracle differs
+from the long-double build by up to 4.0e-11 max_k|Delta_l|, the GPU path by up to 3.2e-11.  With the
+normaliser BASELINE.json states (the largest |Delta_l| over ALL k of the config) both are inside the plain
+1e-10, and that is what the test asserts: no allowance.  (On a subset of the k rows the normaliser is
+smaller: on every 10th row alone the same differences read 1.2e-10, which is why round 1, which compared
+that subset only, carried an allowance.)  The fp64 oracle is run on every k row as well and printed beside
+the GPU figure; DESIGN.md 6.3 carries both, and those of the one variant tried against the floor
+(coefficient carried as hi + lo through the recurrence step: no gain, +27 % time).
 """
 import numpy as np
 import pytest
@@ -188,17 +187,13 @@ def test_config4_extreme(los):
     scale = np.where(scale > 0, scale, 1.0)
     e_gpu = err / scale            # [source][l], over all 20000 k rows
     e_f64 = err64 / scale          # the fp64 floor, same rows, same normaliser
-    win = 512
-    pad = np.pad(e_f64, ((0, 0), (win, win)), mode="edge")
-    floor = np.max(np.lib.stride_tricks.sliding_window_view(pad, 2 * win + 1, axis=1), axis=-1)
     over = e_gpu > TOL_DELTA
     print(f"config 4, all {cfg.n_k} k rows: max Delta error {e_gpu.max():.3e}; l over 1e-10 per source: "
           f"{over.sum(axis=1).tolist()}; fp64 oracle vs long double: max {e_f64.max():.3e}, "
           f"l over 1e-10: {(e_f64 > TOL_DELTA).sum(axis=1).tolist()}")
-    assert np.all(e_gpu <= np.maximum(TOL_DELTA, 2.0 * floor)), "Delta error above 1e-10 and above twice the fp64 floor"
-    assert e_gpu.max() <= max(TOL_DELTA, 1.5 * e_f64.max())
-    assert np.all(e_gpu[2] <= TOL_DELTA)                          # the lensing source is not in that regime
-    assert over.sum() < 0.01 * over.size
+    assert np.all(e_gpu <= TOL_DELTA), "Delta error above 1e-10 max_k|Delta_l|"      # the plain bar of BASELINE.json
+    assert e_gpu.max() <= 1.5 * e_f64.max()                       # and no worse than the fp64 floor of the method
+    assert np.all(e_gpu[2] <= 0.01 * TOL_DELTA)                   # the lensing source is far from that regime
     # below l = 7000 the plain bar holds with margin
     assert np.all(e_gpu[:, : 7000 - cfg.l_min] <= 0.2 * TOL_DELTA)
 
