@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(CLS_THREADS) cls_kernel(const double *__restri
 // ---- streaming kernel (TMA bulk copies into a shared-memory ring)
 constexpr int CLS_STREAM_MAX_K = 6144;    // weights of one cosmology in shared memory: 48 KB
 constexpr int CLS_STREAM_CHUNK = 1536;    // k per ring stage and source: 12 KB
-constexpr int CLS_STAGES = 4;
+__host__ __device__ constexpr int cls_stages(int n_src) { return n_src == 2 ? 6 : 4; }   // ring depth: 144 KB of Delta in flight per SM
 constexpr int CLS_CONSUMERS = 256;        // + one producer warp
 
 __device__ __forceinline__ void bulk_load(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar)
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(CLS_CONSUMERS + 32, 1) cls_stream_kernel(const
                                                                            double *__restrict__ Cl, int n_l, int n_k,
                                                                            long long n_rows, int KC, int n_chunks, int te_last)
 {
-    constexpr int NSPEC = NSRC + 1, NW = CLS_CONSUMERS / 32;
+    constexpr int NSPEC = NSRC + 1, NW = CLS_CONSUMERS / 32, CLS_STAGES = cls_stages(NSRC);
     extern __shared__ __align__(16) double sm_cls[];
     double *wgt = sm_cls;                                           // [n_k] dlnk P_R of the current cosmology
     double *ring = wgt + ((n_k + 1) & ~1);                          // [STAGES][NSRC][KC]
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(CLS_CONSUMERS + 32, 1) cls_stream_kernel(const
         for (int chunk = 0; chunk < n_chunks; ++chunk, ++it) {
             const int s = (int)(it % CLS_STAGES);
             const int len = min(KC, n_k - chunk * KC);
-            mbar_wait(bar_full + 8 * s, (int)(it / CLS_STAGES) & 1);
+            mbar_wait(bar_full + 8 * s, (int)(it / CLS_STAGES) & 1, 64);   // short naps: the data is on its way
             const double2 *w2 = reinterpret_cast<const double2 *>(wgt + (size_t)chunk * KC);
             const double2 *d2 = reinterpret_cast<const double2 *>(ring + (size_t)s * NSRC * KC);
             for (int j = tid; j < len / 2; j += CLS_CONSUMERS) {
@@ -232,8 +232,8 @@ __global__ void __launch_bounds__(CLS_CONSUMERS + 32, 1) cls_stream_kernel(const
 
 static size_t cls_stream_smem(int n_src, int n_k, int KC)
 {
-    return sizeof(double) * (((size_t)n_k + 1) & ~(size_t)1) + sizeof(double) * (size_t)CLS_STAGES * n_src * KC +
-           sizeof(double) * 2 * (n_src + 1) * (CLS_CONSUMERS / 32) + 8 * 2 * CLS_STAGES;
+    return sizeof(double) * (((size_t)n_k + 1) & ~(size_t)1) + sizeof(double) * (size_t)cls_stages(n_src) * n_src * KC +
+           sizeof(double) * 2 * (n_src + 1) * (CLS_CONSUMERS / 32) + 8 * 2 * cls_stages(n_src);
 }
 
 template <int NSRC, int R, int THREADS>

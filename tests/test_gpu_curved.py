@@ -201,6 +201,58 @@ def test_closed_universe_against_the_oracle(los, case):
     plan.close()
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_random_small_curved_shapes(los, seed):
+    """Seeded random grids, l lists, curvature radii and batch sizes around the kernel's shape boundaries, open
+    (even seeds) and closed (odd seeds) universes, element by element against the long-double oracle; the bar
+    carries the skip rule's own allowance (1e-30 sum |w S|) where Delta_l lies below the cut (cf. the flat test)."""
+    rng = np.random.default_rng(5000 + seed)
+    closed = bool(seed % 2)
+    tau0 = 14000.0
+    n_tau = int(rng.choice([2, 3, 32, 33, 127, 129, 300, 641, 1537, 2600]))
+    tau = np.unique(np.sort(rng.uniform(10.0, 13990.0, n_tau)))
+    r_c = float(rng.choice([9500.0, 12000.0, 20000.0, 60000.0])) if closed else float(rng.choice([5000.0, 9000.0, 20000.0, 3.0e5]))
+    n_k = int(rng.integers(2, 12))
+    if closed:
+        beta = np.unique(rng.integers(3, int(rng.choice([40, 400, 4000])), n_k))
+        k = beta / r_c
+        K = 1.0 / r_c ** 2
+    else:
+        k = np.unique(np.sort(float(rng.choice([1e-3, 0.02, 0.2])) * rng.uniform(1e-3, 1.0, n_k)))
+        K = -1.0 / r_c ** 2
+    n_k = k.size
+    if n_k < 2:
+        pytest.skip("degenerate draw")
+    with_phi = bool(rng.integers(0, 2))
+    B = int(rng.choice([1, 1, 2, 3]))
+    l_lo = int(rng.choice([2, 2, 17, 300]))
+    l_all = np.arange(l_lo, l_lo + int(rng.choice([0, 1, 7, 8, 9, 63, 200])) + 1)
+    if rng.integers(0, 2) and l_all.size > 3:
+        l_all = np.sort(rng.choice(l_all, size=max(2, l_all.size // int(rng.integers(2, 9))), replace=False))
+    l_list = l_all.astype(np.int32)
+    S = rng.standard_normal((3, B, n_k, tau.size)) * np.exp(rng.uniform(-20, 5, (3, B, n_k, 1)))
+    plan = los.Plan(l_list, k, tau, tau0, with_phi=with_phi, curvature_K=K)
+    n_src = 3 if with_phi else 2
+    D = torch.full((B, n_src, l_list.size, n_k), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer_batched(dev(S[0]), dev(S[1]), dev(S[2]) if with_phi else None, out=D)
+    torch.cuda.synchronize()
+    D = D.cpu().numpy()
+    w = oracle.trapz_weights(tau)
+    chi = (tau0 - tau) / r_c
+    bs = (k * r_c)[:, None] * (np.sin(chi) if closed else np.sinh(chi))[None, :]
+    pref = np.sqrt((l_list + 2.0) * (l_list + 1.0) * l_list * (l_list - 1.0))
+    for c in range(B):
+        D_ref = oracle.transfer_curved(l_list, k, tau, tau0, K, S[0, c], S[1, c], S[2, c] if with_phi else None, real="f80")
+        skip = [np.sum(np.abs(w * S[0, c]), axis=1)[None, :] * np.ones((l_list.size, 1)),
+                np.sum(np.abs(w * S[1, c]) / bs ** 2, axis=1)[None, :] * pref[:, None]]
+        if with_phi:
+            skip.append(np.sum(np.abs(w * S[2, c]), axis=1)[None, :] * np.ones((l_list.size, 1)))
+        bound = TOL_DELTA * np.max(np.abs(D_ref), axis=-1, keepdims=True) + 1e-30 * np.stack(skip)
+        assert np.all(np.isfinite(D[c]))
+        assert np.all(np.abs(D[c] - D_ref) <= bound), (seed, closed, tau.size, n_k, with_phi, B, r_c, l_list[0], l_list[-1])
+    plan.close()
+
+
 def test_curved_plans_that_are_rejected(los):
     tau = np.linspace(100.0, 13000.0, 10)
     l_list = np.arange(2, 6, dtype=np.int32)
