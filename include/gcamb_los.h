@@ -179,7 +179,7 @@ gcamb_status gcamb_los_cls_batched(const gcamb_los_plan *plan, int32_t n_batch,
  * every spectrum alike, C_l = y(l) / (l (l+1)) afterwards.  The listed multipoles come back
  * unchanged up to rounding (y_i / (l_i (l_i+1))).  The LU factors of the spline's tridiagonal system
  * depend on the l list only and are plan tables; a call runs one kernel, one thread block per
- * (cosmology, spectrum).  Needs 2 <= n_l <= 12800 (GCAMB_EINVAL otherwise).
+ * (cosmology, spectrum).  Needs 2 <= n_l <= 10000 (GCAMB_EINVAL otherwise).
  *   d_Cl     DEVICE [n_batch][n_spec][n_l]                     as written by gcamb_los_cls[_batched]
  *   d_Cl_all DEVICE [n_batch][n_spec][l_list[n_l-1] - l_list[0] + 1], one entry per integer l
  * Asynchronous on `cuda_stream`; deterministic.
@@ -224,7 +224,7 @@ gcamb_status gcamb_los_cls_tensor(const gcamb_los_plan *plan, const double *d_De
  *   k_coarse   HOST [n_kc] strictly increasing, > 0; every k of the plan must lie inside
  *              [k_coarse[0], k_coarse[n_kc-1]] (GCAMB_EGRID otherwise: no extrapolation); n_kc >= 2
  *   n_series   number of independent [n_kc][n_tau] arrays (sources x cosmologies), <= 65535
- *   d_S_coarse DEVICE [n_series][n_kc][n_tau];  d_S_fine DEVICE [n_series][n_k][n_tau] (n_k <= 65535)
+ *   d_S_coarse DEVICE [n_series][n_kc][n_tau];  d_S_fine DEVICE [n_series][n_k][n_tau] (n_k <= 524280)
  *   d_work     DEVICE scratch of the size of d_S_coarse (second derivatives of the splines)
  * Asynchronous on `cuda_stream`; two kernels; deterministic.
  */

@@ -125,7 +125,7 @@ gcamb_status launch_fused(const gcamb_los_plan *p, int n_batch, const double *S_
                           const double *P_R, double *scratch, double *Cl, cudaStream_t stream);
 
 // interp.cu: C_l on every integer l of [l_min, l_max] from C_l on the l list (natural cubic spline of l(l+1) C_l)
-constexpr size_t INTERP_SMEM_MAX = 200 * 1024;   // two doubles per knot in shared memory: n_l <= 12800
+constexpr size_t INTERP_SMEM_MAX = 200000;   // two doubles and an int per knot in shared memory: n_l <= 10000
 gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaStream_t stream);
 gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double *Cl_samp, double *Cl_all,
                               cudaStream_t stream);

@@ -111,17 +111,22 @@ __global__ void __launch_bounds__(128) srcinterp_solve_kernel(const double *__re
     }
 }
 
+constexpr int EVAL_ROWS = 8;   // fine k rows per CTA (one row per CTA: 30000 one-shot CTAs, 33 us for 58 MB)
+
 __global__ void __launch_bounds__(256) srcinterp_eval_kernel(const double *__restrict__ S_c, const double *__restrict__ M,
                                                              const int32_t *__restrict__ seg, const double4 *__restrict__ wgt,
                                                              double *__restrict__ S_f, int n_kc, int n_k, int n_tau)
 {
-    const int j = blockIdx.y;
-    const size_t cbase = (size_t)blockIdx.z * n_kc * n_tau, fbase = ((size_t)blockIdx.z * n_k + j) * n_tau;
-    const int s = seg[j];
-    const double4 w = wgt[j];
-    const double *y0 = S_c + cbase + (size_t)s * n_tau, *m0 = M + cbase + (size_t)s * n_tau;
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_tau; t += gridDim.x * blockDim.x)
-        S_f[fbase + t] = w.x * y0[t] + w.y * y0[n_tau + t] + (w.z * m0[t] + w.w * m0[n_tau + t]);
+    const size_t cbase = (size_t)blockIdx.z * n_kc * n_tau;
+    const int j_end = min(n_k, (int)(blockIdx.y + 1) * EVAL_ROWS);
+    for (int j = blockIdx.y * EVAL_ROWS; j < j_end; ++j) {
+        const size_t fbase = ((size_t)blockIdx.z * n_k + j) * n_tau;
+        const int s = seg[j];
+        const double4 w = wgt[j];
+        const double *y0 = S_c + cbase + (size_t)s * n_tau, *m0 = M + cbase + (size_t)s * n_tau;
+        for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_tau; t += gridDim.x * blockDim.x)
+            S_f[fbase + t] = w.x * y0[t] + w.y * y0[n_tau + t] + (w.z * m0[t] + w.w * m0[n_tau + t]);
+    }
 }
 
 }  // namespace
@@ -220,7 +225,7 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *si, int32_t n_s
 {
     if (!si || !d_S_coarse || !d_S_fine || !d_work) { set_error("null handle or buffer"); return GCAMB_EINVAL; }
     if (n_series < 1 || n_series > 65535) { set_error("n_series must be in [1, 65535]"); return GCAMB_EINVAL; }
-    if (si->n_k > 65535) { set_error("n_k above 65535 not supported by the source interpolation"); return GCAMB_EINVAL; }
+    if (si->n_k > 65535 * EVAL_ROWS) { set_error("n_k above 524280 not supported by the source interpolation"); return GCAMB_EINVAL; }
     int dev = -1;
     GCAMB_CUDA(cudaGetDevice(&dev));
     if (dev != si->device) { set_error("handle belongs to device %d but device %d is current", si->device, dev); return GCAMB_EINVAL; }
@@ -238,7 +243,7 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *si, int32_t n_s
         srcinterp_solve_kernel<false><<<g1, threads, 0, s>>>(d_S_coarse, d_work, si->d_h, si->d_ih, si->d_mult, si->d_inv_diag, si->n_kc, si->n_tau);
     }
     GCAMB_CUDA(cudaGetLastError());
-    dim3 g2((unsigned)std::min((si->n_tau + 255) / 256, 16), (unsigned)si->n_k, (unsigned)n_series);
+    dim3 g2((unsigned)std::min((si->n_tau + 255) / 256, 16), (unsigned)((si->n_k + EVAL_ROWS - 1) / EVAL_ROWS), (unsigned)n_series);
     srcinterp_eval_kernel<<<g2, 256, 0, s>>>(d_S_coarse, d_work, si->d_seg, si->d_wgt, d_S_fine, si->n_kc, si->n_k, si->n_tau);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
