@@ -210,6 +210,11 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                                                  (((size_t)T * NT + WM * 2 * T + 1) & ~(size_t)1)) + tid;
     const uint32_t bar_full = (uint32_t)__cvta_generic_to_shared(ring + (size_t)RD * G * WM * P);
     const uint32_t bar_empty = bar_full + 8 * RD;
+    // open / closed universes only: this warp's copy of the coefficient pairs of two ring groups [2][G V]
+    // (double-buffered: the pairs of group n + 1 are fetched with cp.async while group n is walked; read
+    // straight from global memory every tile they cost an L2 round trip per tile: long_scoreboard 1.2 per issue)
+    double2 *cfs = reinterpret_cast<double2 *>(reinterpret_cast<int *>(ring + (size_t)RD * G * WM * P + 2 * RD) +
+                                               (((size_t)T * NT + WM * 2 * T + 3) & ~(size_t)3)) + (size_t)warp * 2 * G * V;
     if (tid == 0) for (int d = 0; d < 2 * RD; ++d) mbar_init(bar_full + 8 * d, W);
     __syncthreads();
     const int bid = blockIdx.x;
@@ -402,6 +407,25 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         g_any = !SPARSE;
         if (n >= RD) mbar_wait(bar_empty + 8 * (n % RD), ((n / RD) - 1) & 1);
         const int gcount = min(G, n_walk - n * G);
+        if constexpr (CURVED) {
+            auto fetch_group = [&](int m) {   // coefficient pairs of group m -> buffer m & 1 (16 bytes per cp.async)
+                const int cnt = min(G, n_walk - m * G) * V;
+                const double2 *src = p.coef + ((size_t)kidx * p.n_tiles + t_begin + (size_t)m * G) * V;
+                for (int i = lane; i < cnt; i += 32) {
+                    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(cfs + (m & 1) * G * V + i);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + i) : "memory");
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+            };
+            if (n == 0) fetch_group(0);
+            if (n + 1 < n_groups) {
+                fetch_group(n + 1);
+                asm volatile("cp.async.wait_group 1;" ::: "memory");   // group n has landed, n + 1 may be in flight
+            } else {
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+            }
+            __syncwarp();
+        }
         for (int g = 0; g < gcount; ++g, ++t, tl0 -= 2.0 * V) {
         while (next_slot <= t) {
             ++na;
@@ -445,9 +469,9 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                 for (int s = 0; s < V; ++s) acc[q][s] = 0.0;
             double2 cf[V];   // open universe: the tile's V coefficient pairs (the same for every thread of the CTA)
             if constexpr (CURVED) {
-                const double2 *cp = p.coef + ((size_t)kidx * p.n_tiles + t) * V;
+                const double2 *cp = cfs + (n & 1) * G * V + g * V;
 #pragma unroll
-                for (int s = 0; s < V; ++s) cf[s] = __ldg(cp + s);
+                for (int s = 0; s < V; ++s) cf[s] = cp[s];
             }
 #define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C, CURVED>(tl0, cf, ix, my_ixlo, NT, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
@@ -549,6 +573,7 @@ static gcamb_status launch_impl(TransferParams prm, const TransferShape &sh, int
                       sizeof(double) * (RD * RING_G * W * NSRC * V + 2 * RD) +
                       sizeof(int) * (((size_t)T * threads + W * 2 * T + 1) & ~(size_t)1);
         if (COMP) smem += sizeof(double) * T * threads;
+        if (CURVED) smem += sizeof(double2) * W * 2 * RING_G * V + 16;   // coefficient staging (after the 16-byte aligned int tables)
         return smem;
     };
     // register budget: per-thread state is T x (3 + NSRC) + NSRC x V doubles; CTAs of <= 128 threads
