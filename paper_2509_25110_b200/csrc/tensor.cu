@@ -15,8 +15,9 @@
 // tau-sum, reduction), so the tensor path is two runs of the three-source kernels of transfer.cu on a
 // plan whose l list is the union of {l} and {l + 1}, fed with
 //   run A: (S_E, S_T, S_E / x) -> (U1, pref W, U3)      run B: (S_B, S_E, S_B / x) -> (V2, pref U2, V1)
-// (the kernel's second slot carries the 1/x^2 weight and the sqrt((l+2)!/(l-2)!) prefactor), a small
-// kernel in front that forms S / x, and a small kernel behind that combines the rows.  10 FP64
+// (the kernel's second slot carries the 1/x^2 weight and the sqrt((l+2)!/(l-2)!) prefactor), issued as one
+// batched launch of two members, with a small kernel in front that lays the sources out (and forms S / x) and
+// a small kernel behind that combines the rows.  10 FP64
 // instructions per executed (l, k, tau) term against the 8 a dedicated six-sum kernel would need; tensor
 // runs are small (l_max_tensor = 1500 against l_max_scalar = 11000).
 #include <algorithm>
@@ -27,15 +28,19 @@ namespace gcamb {
 
 namespace {
 
-// S_E / x and S_B / x with the plan's correctly rounded 1/x
-__global__ void __launch_bounds__(256) tensor_prep_kernel(const double *__restrict__ S_E, const double *__restrict__ S_B,
-                                                          const double *__restrict__ inv_x,
-                                                          double *__restrict__ SEx, double *__restrict__ SBx, size_t n)
+// The two runs go out as ONE batched launch (twice the thread blocks: a finer tail than two launches of n_k
+// blocks each), so their sources are laid out as a batch of two per kernel slot:
+//   slot 0 = [S_E | S_B],  slot 1 = [S_T | S_E],  slot 2 = [S_E / x | S_B / x]   (1/x: the plan's rounded reciprocal)
+__global__ void __launch_bounds__(256) tensor_prep_kernel(const double *__restrict__ S_T, const double *__restrict__ S_E,
+                                                          const double *__restrict__ S_B, const double *__restrict__ inv_x,
+                                                          double *__restrict__ slot0, double *__restrict__ slot1,
+                                                          double *__restrict__ slot2, size_t n)
 {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const double inv = inv_x[i];
-        SEx[i] = S_E[i] * inv;
-        SBx[i] = S_B[i] * inv;
+        const double inv = inv_x[i], t = S_T[i], e = S_E[i], b = S_B[i];
+        slot0[i] = e;       slot0[n + i] = b;
+        slot1[i] = t;       slot1[n + i] = e;
+        slot2[i] = e * inv; slot2[n + i] = b * inv;
     }
 }
 
@@ -62,20 +67,19 @@ __global__ void __launch_bounds__(256) tensor_combine_kernel(const double *__res
 
 size_t tensor_work_bytes(const gcamb_los_plan *p)
 {
-    return sizeof(double) * (2 * (size_t)p->n_k * p->n_tau + 6 * (size_t)p->n_l * p->n_k);
+    return sizeof(double) * (6 * (size_t)p->n_k * p->n_tau + 6 * (size_t)p->n_l * p->n_k);
 }
 
 gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, const double *S_T, const double *S_E, const double *S_B,
                                     double *Delta, double *work, cudaStream_t stream)
 {
     const size_t n_pt = (size_t)p->n_k * p->n_tau, n_raw = 3 * (size_t)p->n_l * p->n_k;
-    double *SEx = work, *SBx = work + n_pt, *rawA = work + 2 * n_pt, *rawB = rawA + n_raw;
+    double *slot0 = work, *slot1 = work + 2 * n_pt, *slot2 = work + 4 * n_pt, *rawA = work + 6 * n_pt, *rawB = rawA + n_raw;
     const unsigned blocks = (unsigned)std::min<size_t>((n_pt + 255) / 256, (size_t)p->n_sm * 16);
-    tensor_prep_kernel<<<blocks, 256, 0, stream>>>(S_E, S_B, p->d_inv, SEx, SBx, n_pt);
+    tensor_prep_kernel<<<blocks, 256, 0, stream>>>(S_T, S_E, S_B, p->d_inv, slot0, slot1, slot2, n_pt);
     GCAMB_CUDA(cudaGetLastError());
-    gcamb_status st = launch_transfer(p, 1, S_E, S_T, SEx, rawA, stream);
-    if (st != GCAMB_OK) return st;
-    st = launch_transfer(p, 1, S_B, S_E, SBx, rawB, stream);
+    // batch member 0 = run A -> rawA, member 1 = run B -> rawB (contiguous: [2][3][n_le][n_k])
+    gcamb_status st = launch_transfer(p, 2, slot0, slot1, slot2, rawA, stream);
     if (st != GCAMB_OK) return st;
     dim3 grid((unsigned)std::min((p->n_k + 255) / 256, 64), (unsigned)p->n_l_out);
     tensor_combine_kernel<<<grid, 256, 0, stream>>>(rawA, rawB, p->d_t_pos0, p->d_t_pos1, p->d_t_cE, p->d_t_cB,
