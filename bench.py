@@ -47,7 +47,7 @@ NCU_TRAFFIC_BYTES = {
     0: 5.308e6,
     1: (155.7e6 + 91.24e6) + 3.062e6,
     2: (1.466e9 + 1.327e9) + (0.09813e9 + 0.04122e9),
-    3: (5.63e9 + 2.026e9) + (0.5682e9 + 0.006468e9),
+    3: (5.604e9 + 2.034e9) + (0.5681e9 + 0.007168e9),
     4: (3.948e9 + 4.605e9) + (0.4554e9 + 0.7074e9),
 }
 
