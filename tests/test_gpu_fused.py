@@ -109,6 +109,42 @@ def test_fused_with_a_sparse_l_list(los):
     plan.close()
 
 
+def test_emulator_step_captures_into_a_cuda_graph(los):
+    """SURVEY 8(f) NEXT-1, second half: the whole batched step (fused kernel, finish kernel, spline to every l)
+    only enqueues work on the caller's stream, so an emulator loop captures it once and replays it on new
+    sources written into the same buffers."""
+    cfg = synth.Config(9, "fused-graph", 2, 700, 30, 1e-4, 0.3, 150, 80, False, n_batch=8)
+    l_list = np.unique(np.concatenate([np.arange(2, 20), np.arange(20, 100, 10), np.arange(100, 701, 50)])).astype(np.int32)
+    hS, hP = batch_inputs(cfg)
+    plan = los.Plan(l_list, cfg.k(), cfg.tau(), cfg.tau0)
+    assert plan.gcamb_los_spectra_batched_info(8)["fused"]
+    d_T, d_E, d_P = dev(hS[0]), dev(hS[1]), dev(hP)
+    C = torch.empty(8, 3, l_list.size, dtype=torch.float64, device="cuda")
+    C_all = torch.empty(8, 3, 699, dtype=torch.float64, device="cuda")
+    plan.gcamb_los_spectra_batched(d_T, d_E, None, d_P, out=C)           # first call: one-time function attributes
+    plan.gcamb_los_cl_interp(C, out=C_all)
+    torch.cuda.synchronize()
+    C0, C_all0 = C.clone(), C_all.clone()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            plan.gcamb_los_spectra_batched(d_T, d_E, None, d_P, out=C)
+            plan.gcamb_los_cl_interp(C, out=C_all)
+    for _ in range(2):
+        C.fill_(float("nan"))
+        C_all.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(C, C0) and torch.equal(C_all, C_all0)
+    # new cosmologies in the same buffers: the replay computes what a direct call computes
+    perm = torch.tensor([3, 0, 7, 1, 6, 2, 5, 4], device="cuda")
+    d_T.copy_(d_T[perm].clone()); d_E.copy_(d_E[perm].clone()); d_P.copy_(d_P[perm].clone())
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(C, C0[perm]) and torch.equal(C_all, C_all0[perm])
+    plan.close()
+
+
 @pytest.mark.parametrize("case", ["phi", "single", "long_tau"])
 def test_plans_outside_the_fused_kernel_take_the_two_kernel_path(los, case):
     with_phi = case == "phi"
