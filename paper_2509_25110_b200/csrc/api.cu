@@ -439,6 +439,8 @@ gcamb_status gcamb_los_spectra_batched_info(const gcamb_los_plan *plan, int32_t 
 
 }  // extern "C"
 
+constexpr size_t HOST_PIPELINE_MIN_BYTES = 4u << 20;
+
 // everything gcamb_los_spectra_host enqueues; on an error the caller joins the streams before returning
 static gcamb_status spectra_host_enqueue(gcamb_los_plan *p, int32_t n_batch, const double *h_S_T,
                                          const double *h_S_E, const double *h_S_phi, const double *h_P_R,
@@ -467,7 +469,10 @@ static gcamb_status spectra_host_enqueue(gcamb_los_plan *p, int32_t n_batch, con
     // (little to wait for, and its rows carry a third of the work), the last one is half the rows
     // (light ones).  H2D of 8 n_src N_k N_tau bytes bounds the call; compute hides behind it.
     constexpr int NCH = 4;
-    const bool pipelined = p->order_reversed && p->n_k >= 64;
+    // (below HOST_PIPELINE_MIN_BYTES of sources the ~40 stream and event calls of the pipeline cost more than
+    // the overlap returns: config 0, 1.9 MB, 136 us pipelined)
+    const bool pipelined = p->order_reversed && p->n_k >= 64 &&
+                           sizeof(double) * nS * n_batch * p->n_src >= HOST_PIPELINE_MIN_BYTES;
     if (pipelined && !p->h_streams_ready) {
         GCAMB_CUDA(cudaStreamCreateWithFlags(&p->h_copy, cudaStreamNonBlocking));
         GCAMB_CUDA(cudaEventCreateWithFlags(&p->h_start, cudaEventDisableTiming));

@@ -294,9 +294,10 @@ def test_host_buffer_entry_point_matches_device_path(los):
 
 @pytest.mark.parametrize("with_phi", [False, True])
 def test_pipelined_host_entry_point_batched(los, with_phi):
-    """n_k >= 64: the sources go up in four blocks of k rows that overlap the kernels of the blocks
-    before them; results must equal the device-resident path bit for bit, for a batch too."""
-    cfg = synth.Config(9, "mini-pipe", 2, 400, 150, 1e-4, 0.25, 100, 60, with_phi, n_batch=3)
+    """n_k >= 64 and at least 4 MiB of sources: the sources go up in four blocks of k rows that overlap the
+    kernels of the blocks before them; results must equal the device-resident path bit for bit, for a batch too."""
+    cfg = synth.Config(9, "mini-pipe", 2, 400, 300, 1e-4, 0.25, 250, 150, with_phi, n_batch=3)
+    assert 8 * cfg.n_k * cfg.n_tau * cfg.n_batch * (3 if with_phi else 2) >= 4 << 20
     plan = los.Plan(cfg.l_list(), cfg.k(), cfg.tau(), cfg.tau0, with_phi=with_phi)
     S = [synth.sources(cfg, c) for c in range(cfg.n_batch)]
     hS = [np.stack([s[q] for s in S]) if S[0][q] is not None else None for q in range(3)]
