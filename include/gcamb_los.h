@@ -201,9 +201,13 @@ gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, co
  * P_t).  `plan` must have been created with src_mask = GCAMB_SRC_TENSOR.  The transfer call runs the
  * three-source transfer kernels twice on the union of {l} and {l + 1} (the E and B kernels are
  * combinations of plain j_l and j_{l+1} sums with l-dependent coefficients) plus two small kernels; it
- * needs caller-owned scratch of gcamb_los_tensor_work_bytes() bytes.  Single cosmology.
+ * needs caller-owned scratch of gcamb_los_tensor_work_bytes() bytes PER COSMOLOGY.
  *   d_S_T, d_S_E, d_S_B DEVICE [n_k][n_tau];  d_Delta DEVICE [3][n_l][n_k], order T, E, B;
  *   d_work DEVICE scratch;  d_P_t DEVICE [n_k];  d_Cl DEVICE [4][n_l], order TT, EE, BB, TE.
+ * The *_batched forms take n_batch cosmologies on one plan (a5; emulator use-case PAPER.md:24, 248), every
+ * array with a leading [n_batch] dimension and n_batch * gcamb_los_tensor_work_bytes() bytes of scratch:
+ * ONE launch of the transfer kernels with 2 n_batch members; results equal a loop of single calls bit for
+ * bit.  1 <= n_batch <= 32767 (transfer), 65535 (cls), 2 n_k n_batch < 2^31: GCAMB_EINVAL otherwise.
  * Asynchronous on `cuda_stream`; deterministic.
  */
 gcamb_status gcamb_los_tensor_work_bytes(const gcamb_los_plan *plan, int64_t *bytes);
@@ -212,6 +216,11 @@ gcamb_status gcamb_los_transfer_tensor(const gcamb_los_plan *plan, const double 
                                        void *cuda_stream);
 gcamb_status gcamb_los_cls_tensor(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_t,
                                   double *d_Cl, void *cuda_stream);
+gcamb_status gcamb_los_transfer_tensor_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,
+                                               const double *d_S_E, const double *d_S_B, double *d_Delta,
+                                               double *d_work, void *cuda_stream);
+gcamb_status gcamb_los_cls_tensor_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Delta,
+                                          const double *d_P_t, double *d_Cl, void *cuda_stream);
 
 /*
  * InterpolateSources (SourceToTransfers "begins by calling IntegrationVars_init ... and

@@ -369,23 +369,42 @@ gcamb_status gcamb_los_tensor_work_bytes(const gcamb_los_plan *plan, int64_t *by
     return GCAMB_OK;
 }
 
-gcamb_status gcamb_los_transfer_tensor(const gcamb_los_plan *plan, const double *d_S_T, const double *d_S_E,
-                                       const double *d_S_B, double *d_Delta, double *d_work, void *cuda_stream)
+gcamb_status gcamb_los_transfer_tensor_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_S_T,
+                                               const double *d_S_E, const double *d_S_B, double *d_Delta,
+                                               double *d_work, void *cuda_stream)
 {
     if (!plan || !d_S_T || !d_S_E || !d_S_B || !d_Delta || !d_work) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
     if (!plan->tensor) { set_error("not a tensor plan (create it with GCAMB_SRC_TENSOR)"); return GCAMB_EINVAL; }
+    if (n_batch < 1 || n_batch > 32767) { set_error("n_batch must be in [1, 32767] for tensor plans"); return GCAMB_EINVAL; }
+    if (2LL * plan->n_k * n_batch > 0x7fffffffLL) {   // one CTA per (k, run, cosmology) along grid.x
+        set_error("2 * n_k * n_batch must be below 2^31");
+        return GCAMB_EINVAL;
+    }
     if (gcamb_status st = check_device(plan)) return st;
-    return launch_transfer_tensor(plan, d_S_T, d_S_E, d_S_B, d_Delta, d_work, (cudaStream_t)cuda_stream);
+    return launch_transfer_tensor(plan, n_batch, d_S_T, d_S_E, d_S_B, d_Delta, d_work, (cudaStream_t)cuda_stream);
+}
+
+gcamb_status gcamb_los_transfer_tensor(const gcamb_los_plan *plan, const double *d_S_T, const double *d_S_E,
+                                       const double *d_S_B, double *d_Delta, double *d_work, void *cuda_stream)
+{
+    return gcamb_los_transfer_tensor_batched(plan, 1, d_S_T, d_S_E, d_S_B, d_Delta, d_work, cuda_stream);
+}
+
+gcamb_status gcamb_los_cls_tensor_batched(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Delta,
+                                          const double *d_P_t, double *d_Cl, void *cuda_stream)
+{
+    if (!plan || !d_Delta || !d_P_t || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
+    if (!plan->tensor) { set_error("not a tensor plan (create it with GCAMB_SRC_TENSOR)"); return GCAMB_EINVAL; }
+    if (n_batch < 1 || n_batch > 65535) { set_error("n_batch must be in [1, 65535]"); return GCAMB_EINVAL; }
+    if (gcamb_status st = check_device(plan)) return st;
+    // Eq. 1 on (T, E, B): the scalar kernels' (TT, EE, TE, third-source auto) written in the order TT, EE, BB, TE
+    return launch_cls(plan, n_batch, d_Delta, d_P_t, d_Cl, (cudaStream_t)cuda_stream);
 }
 
 gcamb_status gcamb_los_cls_tensor(const gcamb_los_plan *plan, const double *d_Delta, const double *d_P_t,
                                   double *d_Cl, void *cuda_stream)
 {
-    if (!plan || !d_Delta || !d_P_t || !d_Cl) { set_error("null plan or buffer"); return GCAMB_EINVAL; }
-    if (!plan->tensor) { set_error("not a tensor plan (create it with GCAMB_SRC_TENSOR)"); return GCAMB_EINVAL; }
-    if (gcamb_status st = check_device(plan)) return st;
-    // Eq. 1 on (T, E, B): the scalar kernels' (TT, EE, TE, third-source auto) written in the order TT, EE, BB, TE
-    return launch_cls(plan, 1, d_Delta, d_P_t, d_Cl, (cudaStream_t)cuda_stream);
+    return gcamb_los_cls_tensor_batched(plan, 1, d_Delta, d_P_t, d_Cl, cuda_stream);
 }
 
 gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, const double *d_Cl,

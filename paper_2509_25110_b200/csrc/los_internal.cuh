@@ -132,8 +132,8 @@ gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double
 
 // tensor.cu: tensor-mode transfer functions from two runs of the three-source transfer kernels
 size_t tensor_work_bytes(const gcamb_los_plan *p);
-gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, const double *S_T, const double *S_E, const double *S_B,
-                                    double *Delta, double *work, cudaStream_t stream);
+gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
+                                    const double *S_B, double *Delta, double *work, cudaStream_t stream);
 
 // cls.cu (tensor plans: rows of n_l_out multipoles, spectra written in the order TT, EE, BB, TE)
 gcamb_status launch_cls(const gcamb_los_plan *p, int n_batch, const double *Delta,

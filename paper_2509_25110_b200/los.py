@@ -24,6 +24,7 @@ EXPORTS = (
     "gcamb_los_cls", "gcamb_los_transfer_batched", "gcamb_los_cls_batched", "gcamb_los_spectra_host",
     "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
     "gcamb_los_tensor_work_bytes", "gcamb_los_transfer_tensor", "gcamb_los_cls_tensor",
+    "gcamb_los_transfer_tensor_batched", "gcamb_los_cls_tensor_batched",
     "gcamb_los_srcinterp_create", "gcamb_los_srcinterp_destroy", "gcamb_los_interp_sources",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
@@ -69,6 +70,8 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_tensor_work_bytes.argtypes = [_vp, ctypes.POINTER(_i64)]
     lib.gcamb_los_transfer_tensor.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.gcamb_los_cls_tensor.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_transfer_tensor_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_cls_tensor_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     lib.gcamb_los_srcinterp_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _i32, _vp]
     lib.gcamb_los_srcinterp_destroy.argtypes = [_vp]
     lib.gcamb_los_interp_sources.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
@@ -215,6 +218,30 @@ class Plan:
         _check(load_library().gcamb_los_cls_tensor(
             self._h, _dev(Delta, (3, self.n_l, self.n_k), "Delta"), _dev(P_t, (self.n_k,), "P_t"),
             _dev(out, (4, self.n_l), "Cl"), _stream()))
+        return out
+
+    def gcamb_los_transfer_tensor_batched(self, S_T, S_E, S_B, out=None, work=None) -> torch.Tensor:
+        """Tensor sources [B][n_k][n_tau] x 3 -> Delta [B][3][n_l][n_k]; scratch of B x gcamb_los_tensor_work_bytes()."""
+        B = S_T.shape[0]
+        sh = (B, self.n_k, self.n_tau)
+        if out is None:
+            out = torch.empty((B, 3, self.n_l, self.n_k), dtype=torch.float64, device=S_T.device)
+        n_work = B * (self.gcamb_los_tensor_work_bytes() // 8)
+        if work is None:
+            work = torch.empty(n_work, dtype=torch.float64, device=S_T.device)
+        _check(load_library().gcamb_los_transfer_tensor_batched(
+            self._h, B, _dev(S_T, sh, "S_T"), _dev(S_E, sh, "S_E"), _dev(S_B, sh, "S_B"),
+            _dev(out, (B, 3, self.n_l, self.n_k), "Delta"), _dev(work, (n_work,), "work"), _stream()))
+        return out
+
+    def gcamb_los_cls_tensor_batched(self, Delta, P_t, out=None) -> torch.Tensor:
+        """Delta [B][3][n_l][n_k], P_t [B][n_k] -> C_l [B][4][n_l] (TT, EE, BB, TE)."""
+        B = Delta.shape[0]
+        if out is None:
+            out = torch.empty((B, 4, self.n_l), dtype=torch.float64, device=Delta.device)
+        _check(load_library().gcamb_los_cls_tensor_batched(
+            self._h, B, _dev(Delta, (B, 3, self.n_l, self.n_k), "Delta"), _dev(P_t, (B, self.n_k), "P_t"),
+            _dev(out, (B, 4, self.n_l), "Cl"), _stream()))
         return out
 
     def gcamb_los_cl_interp(self, Cl, out=None) -> torch.Tensor:

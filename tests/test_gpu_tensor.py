@@ -142,6 +142,40 @@ def test_tensor_at_the_papers_tensor_grid_sizes(los):
     plan_s.close()
 
 
+def test_tensor_batched_equals_a_loop_of_single_calls(los):
+    """a5 for the tensor calls: B cosmologies on one plan go out as ONE launch of the transfer kernels with 2 B
+    members; Delta and C_l equal a loop of single calls bit for bit, and the oracle within the bars."""
+    l_list = np.array([2, 3, 4, 9, 10, 30, 31, 32, 77, 150, 151, 260], dtype=np.int32)
+    k = synth.k_grid(45, 1e-4, 0.04)
+    tau = synth.tau_grid(150, 83, TAU0)
+    B = 3
+    S = [tensor_sources(k, tau, seed=77 + c) for c in range(B)]
+    hS = [np.stack([S[c][q] for c in range(B)]) for q in range(3)]
+    hP = np.stack([2.1e-10 * (1.0 + 0.1 * c) * (k / 0.05) ** (-0.01 * (c + 1)) for c in range(B)])
+    plan = los.Plan(l_list, k, tau, TAU0, tensor=True)
+    D = torch.full((B, 3, plan.n_l, plan.n_k), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_transfer_tensor_batched(dev(hS[0]), dev(hS[1]), dev(hS[2]), out=D)
+    C = plan.gcamb_los_cls_tensor_batched(D, dev(hP))
+    torch.cuda.synchronize()
+    assert C.shape == (B, 4, plan.n_l)
+    for c in range(B):
+        D1 = plan.gcamb_los_transfer_tensor(dev(S[c][0]), dev(S[c][1]), dev(S[c][2]))
+        C1 = plan.gcamb_los_cls_tensor(D1, dev(hP[c]))
+        assert torch.equal(D1, D[c]) and torch.equal(C1, C[c])
+    D_ref = oracle.transfer_tensor(l_list, k, tau, TAU0, *S[2], real="f80")
+    assert np.all(delta_err(D[2].cpu().numpy(), D_ref) <= TOL_DELTA)
+    e_auto, e_te = cl_err(C[2].cpu().numpy(), oracle.cls_tensor(k, D_ref, hP[2], real="f80"))
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+    # spectra of the batch on every l (reading R25)
+    C_all = plan.gcamb_los_cl_interp(C)
+    assert C_all.shape == (B, 4, 259)
+    assert torch.equal(C_all[1], plan.gcamb_los_cl_interp(C[1].contiguous()))
+    with pytest.raises(ValueError):                                # scratch of one cosmology for three
+        plan.gcamb_los_transfer_tensor_batched(dev(hS[0]), dev(hS[1]), dev(hS[2]),
+                                               work=torch.zeros(plan.gcamb_los_tensor_work_bytes() // 8, dtype=torch.float64, device="cuda"))
+    plan.close()
+
+
 def test_scalar_and_tensor_calls_do_not_mix(los):
     k = synth.k_grid(8, 1e-4, 0.01)
     tau = np.linspace(100.0, 13000.0, 40)
