@@ -123,8 +123,9 @@ constexpr int LAG = 1;   // a group is flushed this many groups after it was wri
 
 // a2 + a3 for one l-tile and the first NA slots of this thread: NA independent recurrence chains.
 // Slots are taken one after the other (j outer, l inner): the V recurrence steps of a slot form
-// one dependent DFMA chain (8 cycles each, measured), which the 4-5 FP64 instructions of a step
-// and the other resident warps cover, and consecutive instructions share operands.
+// one dependent chain (DMUL + DFMA per step on the plain rows, 8 cycles each, measured), which the
+// other slots' instructions and the other resident warps cover; ptxas interleaves the slots (l
+// outer) whatever the source order, which is what lets consecutive instructions share operands.
 //
 // COMP (reading R14): c = (2l+1) * fl(1/x) carries the relative
 // error r of the rounded reciprocal into EVERY step with the same sign, i.e. the walk follows
@@ -134,7 +135,7 @@ constexpr int LAG = 1;   // a group is flushed this many groups after it was wri
 // far below an ulp of c), which makes c the correctly rounded quotient.
 // CURVED (open universe, reading R28): the step is Phi_{l-1} = A_l coth(chi) Phi_l - R_l Phi_{l+1} with the
 // per-(k, l) coefficients cf[s] = (A_l, R_l) of the plan and ix = coth(chi): one DMUL more per term.
-template <int NA, int T, int V, int NSRC, bool COMP, bool CURVED>
+template <int NA, int T, int V, int NSRC, bool COMP, bool CURVED, bool QFORM>
 __device__ __forceinline__ void tile_body(double tl0, const double2 (&cf)[V], const double (&ix)[T], const double *ixlo, int stride,
                                           const double (&src)[NSRC][T], double (&fa)[T], double (&fb)[T],
                                           double (&acc)[NSRC][V])
@@ -146,10 +147,18 @@ __device__ __forceinline__ void tile_body(double tl0, const double2 (&cf)[V], co
 #pragma unroll
         for (int s = 0; s < V; ++s) {
             const double tl = CURVED ? cf[s].x : tl0 - 2.0 * s;   // 2l+1  (curved: (2l+1)/b_l)
-            const double c = COMP ? fma(tl, ix[j], e) : tl * ix[j];
+            // QFORM (plain single-pass rows): the product is taken as (2l+1) * (f_l / x), not as
+            // ((2l+1) / x) * f_l.  The operand the slots share, 2l+1, then sits in the three-operand DFMA,
+            // where the operand cache (.reuse) saves a register fetch, instead of in the two-operand DMUL,
+            // which is at its two cycles anyway (an FP64 instruction costs max(2, register operands
+            // fetched) cycles: profiles/README.md 6.7).  Measured: config 1 -1.3 %, config 2 -0.6 %, sparse
+            // l lists -2.1 %, open universe -1.6 %; the multi-pass kernels of config 4 +0.4 %: they and the
+            // compensated rows keep the coefficient form.
+            const double c = COMP ? fma(tl, ix[j], e) : (QFORM ? ix[j] * fb[j] : tl * ix[j]);
 #pragma unroll
             for (int q = 0; q < NSRC; ++q) acc[q][s] = fma(src[q][j], fb[j], acc[q][s]);
-            const double fn = CURVED ? fma(c, fb[j], -(cf[s].y * fa[j])) : fma(c, fb[j], -fa[j]);
+            const double fa_w = CURVED ? cf[s].y * fa[j] : fa[j];
+            const double fn = QFORM ? fma(tl, c, -fa_w) : fma(c, fb[j], -fa_w);
             fa[j] = fb[j];
             fb[j] = fn;
         }
@@ -160,7 +169,7 @@ __device__ __forceinline__ void tile_body(double tl0, const double2 (&cf)[V], co
 // about every 50th l): only the recurrence walks it, 2 FP64 instructions per term, no accumulators,
 // no reduction.  The NA chains are interleaved (l outer, slot inner): without the accumulates a
 // single slot's 8-step DFMA chain would be latency-bound.
-template <int NA, int T, int V, bool COMP>
+template <int NA, int T, int V, bool COMP, bool QFORM>
 __device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T], const double *ixlo, int stride,
                                                double (&fa)[T], double (&fb)[T])
 {
@@ -174,8 +183,8 @@ __device__ __forceinline__ void tile_body_walk(double tl0, const double (&ix)[T]
         const double tl = tl0 - 2.0 * s;
 #pragma unroll
         for (int j = 0; j < NA; ++j) {
-            const double c = COMP ? fma(tl, ix[j], e[j]) : tl * ix[j];
-            const double fn = fma(c, fb[j], -fa[j]);
+            const double c = COMP ? fma(tl, ix[j], e[j]) : (QFORM ? ix[j] * fb[j] : tl * ix[j]);
+            const double fn = QFORM ? fma(tl, c, -fa[j]) : fma(c, fb[j], -fa[j]);
             fa[j] = fb[j];
             fb[j] = fn;
         }
@@ -455,7 +464,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         double *rb = ring + ((size_t)((n % RD) * G + g) * WM + warp) * P;   // summed by warp index: a fixed order
         GCAMB_ASSERT(g >= 0 && g < G && warp < W && t >= 0 && na <= T && n * G + g == t - t_begin);
         if (SPARSE && !acc_on) {
-#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C>(tl0, ix, my_ixlo, NT, fa, fb); break;
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body_walk<n, T, V, C, !C && !MULTI>(tl0, ix, my_ixlo, NT, fa, fb); break;
             switch (na) {
                 GCAMB_NA(1, COMP) GCAMB_NA(2, COMP) GCAMB_NA(3, COMP) GCAMB_NA(4, COMP) GCAMB_NA(5, COMP) GCAMB_NA(6, COMP)
                 GCAMB_NA(7, COMP) GCAMB_NA(8, COMP) GCAMB_NA(9, COMP) GCAMB_NA(10, COMP) GCAMB_NA(11, COMP) GCAMB_NA(12, COMP)
@@ -473,7 +482,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
 #pragma unroll
                 for (int s = 0; s < V; ++s) cf[s] = cp[s];
             }
-#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C, CURVED>(tl0, cf, ix, my_ixlo, NT, src, fa, fb, acc); break;
+#define GCAMB_NA(n, C) case n: if constexpr (T >= n) tile_body<n, T, V, NSRC, C, CURVED, !C && !MULTI>(tl0, cf, ix, my_ixlo, NT, src, fa, fb, acc); break;
 #define GCAMB_BODIES(C) switch (na) { \
                 GCAMB_NA(1, C) GCAMB_NA(2, C) GCAMB_NA(3, C) GCAMB_NA(4, C) GCAMB_NA(5, C) \
                 GCAMB_NA(6, C) GCAMB_NA(7, C) GCAMB_NA(8, C) GCAMB_NA(9, C) GCAMB_NA(10, C) \
