@@ -246,6 +246,25 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *handle, int32_t
                                       void *cuda_stream);
 
 /*
+ * gcamb_los_interp_sources for callers that cannot allocate device memory (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same two kernels, same arguments and results (bit for
+ * bit), but the scratch is a file-scope `static __device__` array of the library instead of a caller buffer.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   limit      n_series * n_kc * n_tau <= 1048576 doubles (8 MiB; e.g. two sources x 300 coarse k x 1200 tau);
+ *              GCAMB_EINVAL with a message stating both numbers otherwise (use gcamb_los_interp_sources then)
+ *   cost       every GPU that loads the library holds the 8 MiB array until the process exits
+ *   sharing    all calls on a device share the array: calls that may OVERLAP on the GPU (different streams
+ *              without an ordering between them) race on it and are not supported; calls on one stream, or
+ *              ordered by events, are safe.  Nothing in it needs clearing: every element a call reads it has
+ *              written itself, so the contents an earlier call left behind are never used.
+ *   set-up     the first call on a device looks up the array's device address (cudaGetSymbolAddress, with
+ *              that device current) and keeps it; make that first call outside a stream capture.
+ * The handle (gcamb_los_srcinterp_create) is built beforehand, at set-up, like the plan.
+ */
+gcamb_status gcamb_los_interp_sources_noalloc(const gcamb_los_srcinterp *handle, int32_t n_series,
+                                              const double *d_S_coarse, double *d_S_fine, void *cuda_stream);
+
+/*
  * Batched sources -> spectra in one call, WITHOUT the transfer functions ever reaching memory
  * (the emulator-training use-case: 1e5-1e6 spectra on a fixed grid; Eq. 1-3,
  * PAPER.md:50-58).  For plans with the T and E sources only and n_tau <= 2560 this runs ONE fused

@@ -15,6 +15,7 @@
 //   eval:   one thread per (series, k, tau): four coarse values (L2-resident) -> one fine value, the
 //           HBM-bound part (8 n_k n_tau bytes written per series).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <new>
 #include <vector>
@@ -30,6 +31,13 @@ struct gcamb_los_srcinterp {
     int32_t *d_seg;       // [n_k]    coarse interval of every fine k
     double4 *d_wgt;       // [n_k]    (A, B, (A^3-A) h^2/6, (B^3-B) h^2/6)
 };
+
+// Scratch of gcamb_los_interp_sources_noalloc: the second derivatives of the splines, [n_series][n_kc][n_tau]
+// doubles, at most NOALLOC_SCRATCH_DOUBLES of them (8 MiB).  A file-scope device array: every GPU that loads the
+// library holds it until the process exits, and every call on a device shares it.  In HOST code the name is a
+// host-side stand-in, not a device address: the kernels get the address cudaGetSymbolAddress returns (below).
+constexpr size_t NOALLOC_SCRATCH_DOUBLES = (size_t)1 << 20;
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_SCRATCH_DOUBLES];
 
 namespace gcamb {
 
@@ -247,6 +255,44 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *si, int32_t n_s
     srcinterp_eval_kernel<<<g2, 256, 0, s>>>(d_S_coarse, d_work, si->d_seg, si->d_wgt, d_S_fine, si->n_kc, si->n_k, si->n_tau);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
+}
+
+// Device address of g_noalloc_scratch on the current device: looked up once per device (the first call on it),
+// with that device current, and kept.
+static gcamb_status noalloc_scratch_address(int dev, double **out)
+{
+    constexpr int MAX_DEV = 64;
+    static std::atomic<double *> cache[MAX_DEV];
+    double *ptr = (dev >= 0 && dev < MAX_DEV) ? cache[dev].load(std::memory_order_acquire) : nullptr;
+    if (!ptr) {
+        GCAMB_CUDA(cudaGetSymbolAddress((void **)&ptr, g_noalloc_scratch));   // `dev` is current: the caller checked
+        if (!ptr) { set_error("cudaGetSymbolAddress returned a null address for the static scratch"); return GCAMB_ECUDA; }
+        if (dev >= 0 && dev < MAX_DEV) cache[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_interp_sources_noalloc(const gcamb_los_srcinterp *si, int32_t n_series,
+                                              const double *d_S_coarse, double *d_S_fine, void *cuda_stream)
+{
+    if (!si || !d_S_coarse || !d_S_fine) { set_error("null handle or buffer"); return GCAMB_EINVAL; }
+    if (n_series < 1 || n_series > 65535) { set_error("n_series must be in [1, 65535]"); return GCAMB_EINVAL; }
+    const unsigned long long need = (unsigned long long)n_series * (unsigned long long)si->n_kc * (unsigned long long)si->n_tau;
+    if (need > NOALLOC_SCRATCH_DOUBLES) {
+        set_error("gcamb_los_interp_sources_noalloc: n_series * n_kc * n_tau = %llu doubles exceeds the static scratch of "
+                  "%llu doubles (8 MiB): use gcamb_los_interp_sources with caller-owned scratch",
+                  need, (unsigned long long)NOALLOC_SCRATCH_DOUBLES);
+        return GCAMB_EINVAL;
+    }
+    int dev = -1;
+    GCAMB_CUDA(cudaGetDevice(&dev));
+    if (dev != si->device) { set_error("handle belongs to device %d but device %d is current", si->device, dev); return GCAMB_EINVAL; }
+    double *scratch = nullptr;
+    if (gcamb_status st = noalloc_scratch_address(dev, &scratch)) return st;
+    // Nothing in the scratch has to start at zero: the solve kernel writes every element [series][0 .. n_kc-1][tau]
+    // that the evaluation kernel reads, in the same stream order, so what an earlier call left behind is never read.
+    return gcamb_los_interp_sources(si, n_series, d_S_coarse, d_S_fine, scratch, cuda_stream);
 }
 
 }  // extern "C"

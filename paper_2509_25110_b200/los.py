@@ -26,6 +26,7 @@ EXPORTS = (
     "gcamb_los_tensor_work_bytes", "gcamb_los_transfer_tensor", "gcamb_los_cls_tensor",
     "gcamb_los_transfer_tensor_batched", "gcamb_los_cls_tensor_batched",
     "gcamb_los_srcinterp_create", "gcamb_los_srcinterp_destroy", "gcamb_los_interp_sources",
+    "gcamb_los_interp_sources_noalloc",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
 PROBE_LIB_PATH = os.path.join(_HERE, "libgcamb_probe.so")
@@ -75,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_srcinterp_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _i32, _vp]
     lib.gcamb_los_srcinterp_destroy.argtypes = [_vp]
     lib.gcamb_los_interp_sources.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
+    lib.gcamb_los_interp_sources_noalloc.argtypes = [_vp, _i32, _vp, _vp, _vp]
     _lib = lib
     return lib
 
@@ -323,6 +325,16 @@ class SourceInterp:
             self._h, n_series, _dev(S_coarse, lead + (self.n_kc, self.n_tau), "S_coarse"),
             _dev(out, lead + (self.n_k, self.n_tau), "S_fine"), _dev(work, lead + (self.n_kc, self.n_tau), "work"),
             _stream()))
+        return out
+
+    def gcamb_los_interp_sources_noalloc(self, S_coarse, out) -> torch.Tensor:
+        """As gcamb_los_interp_sources, with the library's static device scratch (at most 2^20 doubles of coarse
+        sources): the call allocates nothing, so `out` is the caller's."""
+        lead = tuple(S_coarse.shape[:-2])
+        n_series = int(np.prod(lead)) if lead else 1
+        _check(load_library().gcamb_los_interp_sources_noalloc(
+            self._h, n_series, _dev(S_coarse, lead + (self.n_kc, self.n_tau), "S_coarse"),
+            _dev(out, lead + (self.n_k, self.n_tau), "S_fine"), _stream()))
         return out
 
 
