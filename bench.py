@@ -574,7 +574,7 @@ def run_next(args) -> None:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
         peak_gbs = float(peaks.get("hbm_gbs", 6650.0))
         value, unit, metric = n_f / t_step, "source values/s", "interpolated source values/s (InterpolateSources)"
-        roof = {"bound": "hbm", "kernel": "srcinterp_eval_kernel + srcinterp_solve_kernel", "achieved": bytes_alg / t_step / 1e9,
+        roof = {"bound": "hbm", "kernel": "srcinterp_mma_kernel + srcinterp_eval_kernel", "achieved": bytes_alg / t_step / 1e9,
                 "peak": peak_gbs, "unit": "GB/s", "frac": bytes_alg / t_step / 1e9 / peak_gbs, "traffic": None,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
                 "algorithmic": f"{bytes_alg} bytes per call: 8 (3 n_coarse + n_fine) n_tau n_series"}

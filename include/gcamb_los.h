@@ -236,11 +236,19 @@ gcamb_status gcamb_los_cls_tensor_batched(const gcamb_los_plan *plan, int32_t n_
  *   d_S_coarse DEVICE [n_series][n_kc][n_tau];  d_S_fine DEVICE [n_series][n_k][n_tau] (n_k <= 524280)
  *   d_work     DEVICE scratch of the size of d_S_coarse (second derivatives of the splines)
  * Asynchronous on `cuda_stream`; two kernels; deterministic.
+ * The spline matrix is diagonally dominant, so its inverse is banded to any wanted accuracy: the handle also holds
+ * the rows of the inverse, cut where what is dropped stays below 1e-18 max|S| in a result (a bound), and the solve
+ * runs as independent dot products of ~60 terms per (coarse k, tau).  Grids whose rows stay wide (more than 100
+ * columns on average: spacings that jump by orders of magnitude) or longer than 4096 keep the two sequential
+ * sweeps per (series, tau); gcamb_los_srcinterp_info reports which (band_columns = columns of the widest row of
+ * the banded inverse, 0 = sequential sweeps; any out pointer may be NULL).
  */
 typedef struct gcamb_los_srcinterp gcamb_los_srcinterp;
 gcamb_status gcamb_los_srcinterp_create(gcamb_los_srcinterp **out, const gcamb_los_plan *plan,
                                         const double *k_coarse, int32_t n_kc, void *cuda_stream);
 gcamb_status gcamb_los_srcinterp_destroy(gcamb_los_srcinterp *handle);
+gcamb_status gcamb_los_srcinterp_info(const gcamb_los_srcinterp *handle, int32_t *n_kc, int32_t *n_k, int32_t *n_tau,
+                                      int32_t *band_columns);
 gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *handle, int32_t n_series,
                                       const double *d_S_coarse, double *d_S_fine, double *d_work,
                                       void *cuda_stream);

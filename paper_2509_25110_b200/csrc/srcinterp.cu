@@ -10,13 +10,16 @@
 // The matrix depends on the coarse grid only: its LU factors, and per fine k its interval and the four
 // weights (A, B, (A^3-A) h^2/6, (B^3-B) h^2/6), are tables of the handle, built once on the host.
 // Arrays are [k][tau] with tau fastest, so thread <-> tau makes every access of both kernels coalesced:
-//   solve:  one thread per (series, tau) walks the coarse grid down and up (two dependent FMA chains of
-//           n_kc steps; the loads do not depend on the chain), second derivatives M to scratch;
-//   eval:   one thread per (series, k, tau): four coarse values (L2-resident) -> one fine value, the
+//   solve:  M = A^-1 d with the banded inverse of the spline matrix as a dense contraction on the FP64 tensor
+//           cores (srcinterp_mma_kernel); grids the band does not serve: one thread per (series, tau) walks the
+//           coarse grid down and up (srcinterp_solve_kernel: two dependent FMA chains of n_kc steps);
+//           second derivatives M to scratch;
+//   eval:   one thread per (series, k, two tau): four coarse values (L2-resident) -> one fine value, the
 //           HBM-bound part (8 n_k n_tau bytes written per series).
 #include <algorithm>
 #include <atomic>
 #include <cmath>
+#include <cstdint>
 #include <new>
 #include <vector>
 
@@ -30,6 +33,11 @@ struct gcamb_los_srcinterp {
     double *d_inv_diag;   // [n_kc]   reciprocals of the eliminated diagonal
     int32_t *d_seg;       // [n_k]    coarse interval of every fine k
     double4 *d_wgt;       // [n_k]    (A, B, (A^3-A) h^2/6, (B^3-B) h^2/6)
+    // banded form of the solve (see srcinterp_mma_kernel); n_iblk = 0: the sequential sweeps are used
+    double *d_blk_val;    // A fragments of the banded inverse: per block of 8 rows and k-step, 32 lane-ordered values
+    int32_t *d_blk_off, *d_blk_jlo, *d_blk_ks;   // [n_iblk] offset into d_blk_val, first column, k-steps of 4 columns
+    int32_t *d_grp_j0, *d_grp_kw;                // [n_grp] first row and number of rows of d a thread block needs
+    int32_t n_iblk, n_grp, kw_max, band_max;     // band_max: columns of the widest row
 };
 
 // Scratch of gcamb_los_interp_sources_noalloc: the second derivatives of the splines, [n_series][n_kc][n_tau]
@@ -119,21 +127,141 @@ __global__ void __launch_bounds__(128) srcinterp_solve_kernel(const double *__re
     }
 }
 
+// The spline matrix is tridiagonal and diagonally dominant by a factor 2 in every row, whatever the grid, so the
+// entries of its inverse fall off at least like 2^-|i-j| (Neumann series; 0.27^|i-j| on a nearly uniform grid):
+// M_i = sum_j (A^-1)_ij d_j needs ~30 columns either side of the diagonal, and every (i, tau) is independent of
+// every other, where the two sweeps of the Thomas algorithm are 2400 dependent chains of 300 steps (73 us, bound
+// by the latency of the chain).  The rows of A^-1 are built on the host at creation and cut where the dropped
+// entries, weighted with the largest right-hand side they can meet and the largest weight the evaluation gives
+// M_i, sum to less than 1e-18 max|S| (a bound, not an estimate).
+// With the band, M[8 rows x tau] = A^-1[8 x K] . d[K x tau] (K ~ 72) is a dense contraction: it runs on the FP64
+// tensor cores (mma.sync.m8n8k4.f64), ONE operand load per 256 multiply-adds.  (The same dot products on the plain
+// FP64 pipe, one thread per tau: 75 us, every FMA waits for its two operand loads: long_scoreboard 16 per issue.)
+// Block = MM_WARPS warps x MM_TAU tau: the right-hand sides d_j of the rows the block's bands reach are formed
+// from the coarse sources (coalesced along tau) into shared memory; warp w then takes the 8 rows of "i-block"
+// 4 group + w: A fragments straight from the host-packed table (lane-ordered, zero outside a row's band: one
+// coalesced 256-byte load per k-step, shared through L1 by the warps of all tau), B fragments from shared memory.
+constexpr int MM_WARPS = 4;
+constexpr int MM_TAU = 32;     // tau per block = 4 MMA column tiles per warp
+constexpr int MM_DS = 36;      // row stride of d in shared memory: 4 rows x 8 tau of a B fragment hit distinct banks
+constexpr int MM_KW_MAX = 200; // rows of d a block may need (57.6 KB)
+
+__device__ __forceinline__ void dmma_884(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(32 * MM_WARPS) srcinterp_mma_kernel(const double *__restrict__ S_c, double *__restrict__ M,
+                                                                      const double *__restrict__ ih, const double *__restrict__ blk_val,
+                                                                      const int32_t *__restrict__ blk_off, const int32_t *__restrict__ blk_jlo,
+                                                                      const int32_t *__restrict__ blk_ks, const int32_t *__restrict__ grp_j0,
+                                                                      const int32_t *__restrict__ grp_kw, int n_kc, int n_tau, int n_iblk)
+{
+    extern __shared__ double dsm[];                 // [Kw][MM_DS]
+    // the evaluation kernel behind this one is launched with programmatic stream serialization: its thread blocks
+    // may become resident as soon as every block of this grid has started, and wait (griddepcontrol.wait) for
+    // this grid to complete before they read M
+    asm volatile("griddepcontrol.launch_dependents;");
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tau0 = blockIdx.x * MM_TAU, grp = blockIdx.y;
+    const int wj0 = grp_j0[grp], Kw = grp_kw[grp];
+    const size_t base = (size_t)blockIdx.z * n_kc * n_tau;
+    // right-hand sides d_j = (y_{j+1} - y_j) / h_j - (y_j - y_{j-1}) / h_{j-1}, j = wj0 .. wj0 + Kw - 1; zero outside
+    // the interior rows and past the end of the tau grid (the A fragments are zero there, but 0 x NaN is not)
+    {
+        const int t = tau0 + lane;
+        const bool tv = t < n_tau;
+        const double *y = S_c + base + (tv ? t : 0);
+        auto row = [&](int q) { return (tv && q >= 0 && q < n_kc) ? y[(size_t)q * n_tau] : 0.0; };
+        const int per = (Kw + MM_WARPS - 1) / MM_WARPS;             // a warp takes consecutive rows: one new load per row
+        const int r0 = warp * per, r1 = min(Kw, r0 + per);
+        if (r0 < r1) {
+            double y0 = row(wj0 + r0 - 1), y1 = row(wj0 + r0);
+#pragma unroll 8
+            for (int r = r0; r < r1; ++r) {
+                const int j = wj0 + r;
+                const double y2 = row(j + 1);
+                double d = 0.0;
+                if (tv && j >= 1 && j <= n_kc - 2) d = fma(y2 - y1, __ldg(ih + j), -((y1 - y0) * __ldg(ih + j - 1)));
+                dsm[r * MM_DS + lane] = d;
+                y0 = y1;
+                y1 = y2;
+            }
+        }
+    }
+    __syncthreads();
+    const int b = grp * MM_WARPS + warp;            // this warp's rows: 8 b .. 8 b + 7
+    if (b >= n_iblk) return;
+    const int ks = blk_ks[b], fr = lane >> 2, fc = lane & 3;
+    const double *av = blk_val + blk_off[b] + lane;
+    const double *dp = dsm + (blk_jlo[b] - wj0 + fc) * MM_DS + fr;
+    double D[MM_TAU / 8][2];
+#pragma unroll
+    for (int nt = 0; nt < MM_TAU / 8; ++nt) D[nt][0] = D[nt][1] = 0.0;
+#pragma unroll 4
+    for (int s = 0; s < ks; ++s) {
+        const double a = __ldg(av + 32 * s);        // A[row fr][column 4 s + fc]
+#pragma unroll
+        for (int nt = 0; nt < MM_TAU / 8; ++nt) dmma_884(D[nt], a, dp[4 * s * MM_DS + 8 * nt]);   // B[k fc][tau 8 nt + fr]
+    }
+    // D fragment: row fr, tau 8 nt + 2 fc, + 1.  Rows 0 and n_kc - 1 carry zero coefficients: M_0 = M_{n-1} = 0.
+    const int row = 8 * b + fr;
+    if (row < n_kc) {
+        double *m = M + base + (size_t)row * n_tau;
+#pragma unroll
+        for (int nt = 0; nt < MM_TAU / 8; ++nt) {
+            const int t = tau0 + 8 * nt + 2 * fc;
+            if (t < n_tau) m[t] = D[nt][0];
+            if (t + 1 < n_tau) m[t + 1] = D[nt][1];
+        }
+    }
+}
+
 constexpr int EVAL_ROWS = 8;   // fine k rows per CTA (one row per CTA: 30000 one-shot CTAs, 33 us for 58 MB)
 
+// s(k_j, tau) = A y_s + B y_{s+1} + C M_s + D M_{s+1}.  VEC = 2: two tau per thread through 16-byte loads and stores
+// (n_tau even, buffers 16-byte aligned); the scalar form of the kernel issued 70 instructions per warp and row and
+// was bound by instruction issue (66 % of the issue slots), not by memory.  Both forms do the same operations in
+// the same order on every element.
+__device__ __forceinline__ double spline_value(const double4 &w, double ya, double yb, double ma, double mb)
+{
+    return fma(w.x, ya, w.y * yb) + fma(w.z, ma, w.w * mb);
+}
+
+template <int VEC>
 __global__ void __launch_bounds__(256) srcinterp_eval_kernel(const double *__restrict__ S_c, const double *__restrict__ M,
                                                              const int32_t *__restrict__ seg, const double4 *__restrict__ wgt,
                                                              double *__restrict__ S_f, int n_kc, int n_k, int n_tau)
 {
     const size_t cbase = (size_t)blockIdx.z * n_kc * n_tau;
-    const int j_end = min(n_k, (int)(blockIdx.y + 1) * EVAL_ROWS);
-    for (int j = blockIdx.y * EVAL_ROWS; j < j_end; ++j) {
-        const size_t fbase = ((size_t)blockIdx.z * n_k + j) * n_tau;
-        const int s = seg[j];
-        const double4 w = wgt[j];
-        const double *y0 = S_c + cbase + (size_t)s * n_tau, *m0 = M + cbase + (size_t)s * n_tau;
-        for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_tau; t += gridDim.x * blockDim.x)
-            S_f[fbase + t] = w.x * y0[t] + w.y * y0[n_tau + t] + (w.z * m0[t] + w.w * m0[n_tau + t]);
+    const int j0 = blockIdx.y * EVAL_ROWS, j_end = min(n_k, j0 + EVAL_ROWS);
+    int sg[EVAL_ROWS];
+    double4 w[EVAL_ROWS];
+#pragma unroll
+    for (int u = 0; u < EVAL_ROWS; ++u) {
+        const int j = min(j0 + u, n_k - 1);
+        sg[u] = seg[j];
+        w[u] = wgt[j];
+    }
+    // launched with programmatic stream serialization: everything above overlaps the tail of the solve kernel;
+    // M is complete and visible after this
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    for (int t = (blockIdx.x * blockDim.x + threadIdx.x) * VEC; t < n_tau; t += gridDim.x * blockDim.x * VEC) {
+#pragma unroll
+        for (int u = 0; u < EVAL_ROWS; ++u) {
+            if (j0 + u < j_end) {
+                const size_t c = cbase + (size_t)sg[u] * n_tau + t, f = ((size_t)blockIdx.z * n_k + j0 + u) * n_tau + t;
+                if (VEC == 2) {
+                    const double2 ya = *reinterpret_cast<const double2 *>(S_c + c), yb = *reinterpret_cast<const double2 *>(S_c + c + n_tau);
+                    const double2 ma = *reinterpret_cast<const double2 *>(M + c), mb = *reinterpret_cast<const double2 *>(M + c + n_tau);
+                    *reinterpret_cast<double2 *>(S_f + f) = make_double2(spline_value(w[u], ya.x, yb.x, ma.x, mb.x),
+                                                                         spline_value(w[u], ya.y, yb.y, ma.y, mb.y));
+                } else {
+                    S_f[f] = spline_value(w[u], S_c[c], S_c[c + n_tau], M[c], M[c + n_tau]);
+                }
+            }
+        }
     }
 }
 
@@ -176,6 +304,71 @@ gcamb_status gcamb_los_srcinterp_create(gcamb_los_srcinterp **out, const gcamb_l
         diag[i] -= mult[i] * sub;
     }
     for (int i = 1; i < n_kc - 1; ++i) inv_diag[i] = 1.0 / diag[i];
+    // Banded inverse (srcinterp_mma_kernel).  Row i of A^-1 = the solution of A x = e_i (A is symmetric) through the
+    // factors above, in long double; it is cut on both sides where the dropped entries can add at most 0.5e-18 max|S|
+    // to an interpolated value: |d_j| <= 2 max|S| (1/h_j + 1/h_{j-1}), and M_i enters a value with a weight of at most
+    // 0.385 max(h_{i-1}, h_i)^2 / 6.  Grids whose rows stay wide (average above BAND_MAX_AVG columns: spacings that
+    // jump by orders of magnitude) and very long grids keep the sequential sweeps.
+    constexpr int BAND_MAX_KC = 4096, BAND_MAX_AVG = 100;
+    std::vector<double> ainv;
+    std::vector<double> blk_val;
+    std::vector<int32_t> a_off(n_kc, 0), a_lo(n_kc, 0), a_cnt(n_kc, 0), blk_off, blk_jlo, blk_ks, grp_j0, grp_kw;
+    int kw_max = 0, band_max = 0;
+    bool band_ok = false;
+    if (n_kc >= 3 && n_kc <= BAND_MAX_KC) {
+        std::vector<long double> r(n_kc), x(n_kc);
+        std::vector<double> g(n_kc, 0.0);
+        for (int j = 1; j < n_kc - 1; ++j) g[j] = 2.0 * (ih[j] + ih[j - 1]);
+        bool ok = true;
+        for (int i = 1; i < n_kc - 1 && ok; ++i) {
+            for (int j = 1; j < n_kc - 1; ++j) r[j] = 0.0L;
+            r[i] = 1.0L;
+            for (int j = i + 1; j < n_kc - 1; ++j) r[j] = -(long double)mult[j] * r[j - 1];
+            long double next = 0.0L;
+            for (int j = n_kc - 2; j >= 1; --j) { next = (r[j] - (long double)h[j] / 6.0L * next) / (long double)diag[j]; x[j] = next; }
+            const double hm = std::max(h[i - 1], h[i]);
+            const long double budget = 0.5e-18L / (0.385L * hm * hm / 6.0L);
+            int lo = 1, hi = n_kc - 2;
+            long double tail = 0.0L;
+            while (lo < i && tail + fabsl(x[lo]) * g[lo] <= budget) { tail += fabsl(x[lo]) * g[lo]; ++lo; }
+            tail = 0.0L;
+            while (hi > i && tail + fabsl(x[hi]) * g[hi] <= budget) { tail += fabsl(x[hi]) * g[hi]; --hi; }
+            a_off[i] = (int32_t)ainv.size(); a_lo[i] = lo; a_cnt[i] = hi - lo + 1;
+            band_max = std::max(band_max, hi - lo + 1);
+            for (int j = lo; j <= hi; ++j) ainv.push_back((double)x[j]);
+            if (ainv.size() > (size_t)BAND_MAX_AVG * (size_t)n_kc) ok = false;
+        }
+        if (ok) {
+            // A fragments: block b = rows 8 b .. 8 b + 7, columns jlo_b + 4 s + c; value of lane 4 r + c, zero outside the row's band
+            const int n_iblk = (n_kc + 7) / 8;
+            for (int bk = 0; bk < n_iblk; ++bk) {
+                int jlo = n_kc, jhi = -1;
+                for (int i = std::max(1, 8 * bk); i < std::min(n_kc - 1, 8 * bk + 8); ++i) {
+                    jlo = std::min(jlo, a_lo[i]);
+                    jhi = std::max(jhi, a_lo[i] + a_cnt[i] - 1);
+                }
+                const int ks = jhi >= jlo ? (jhi - jlo + 1 + 3) / 4 : 0;
+                blk_off.push_back((int32_t)blk_val.size()); blk_jlo.push_back(ks ? jlo : 1); blk_ks.push_back(ks);
+                for (int st = 0; st < ks; ++st)
+                    for (int ln = 0; ln < 32; ++ln) {
+                        const int i = 8 * bk + (ln >> 2), jcol = jlo + 4 * st + (ln & 3);
+                        double v = 0.0;
+                        if (i >= 1 && i <= n_kc - 2 && jcol >= a_lo[i] && jcol < a_lo[i] + a_cnt[i]) v = ainv[a_off[i] + (jcol - a_lo[i])];
+                        blk_val.push_back(v);
+                    }
+            }
+            const int n_grp = (n_iblk + MM_WARPS - 1) / MM_WARPS;
+            for (int gq = 0; gq < n_grp; ++gq) {
+                int j0 = n_kc, j1 = 0;
+                for (int bk = gq * MM_WARPS; bk < std::min(n_iblk, (gq + 1) * MM_WARPS); ++bk)
+                    if (blk_ks[bk]) { j0 = std::min(j0, blk_jlo[bk]); j1 = std::max(j1, blk_jlo[bk] + 4 * blk_ks[bk]); }
+                grp_j0.push_back(j1 > j0 ? j0 : 1);
+                grp_kw.push_back(j1 > j0 ? j1 - j0 : 0);
+                kw_max = std::max(kw_max, grp_kw.back());
+            }
+            band_ok = kw_max <= MM_KW_MAX;
+        }
+    }
     std::vector<int32_t> seg(n_k);
     std::vector<double4> wgt(n_k);
     for (int j = 0; j < n_k; ++j) {
@@ -204,6 +397,25 @@ gcamb_status gcamb_los_srcinterp_create(gcamb_los_srcinterp **out, const gcamb_l
     if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_inv_diag, inv_diag.data(), sizeof(double) * n_kc, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_seg, seg.data(), sizeof(int32_t) * n_k, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_wgt, wgt.data(), sizeof(double4) * n_k, cudaMemcpyHostToDevice, s);
+    if (band_ok) {
+        const size_t nb = blk_off.size(), ng = grp_j0.size();
+        si->n_iblk = (int32_t)nb; si->n_grp = (int32_t)ng; si->kw_max = kw_max; si->band_max = band_max;
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_blk_val, sizeof(double) * std::max<size_t>(blk_val.size(), 1));
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_blk_off, sizeof(int32_t) * nb);
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_blk_jlo, sizeof(int32_t) * nb);
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_blk_ks, sizeof(int32_t) * nb);
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_grp_j0, sizeof(int32_t) * ng);
+        if (e == cudaSuccess) e = cudaMalloc(&si->d_grp_kw, sizeof(int32_t) * ng);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_blk_val, blk_val.data(), sizeof(double) * blk_val.size(), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_blk_off, blk_off.data(), sizeof(int32_t) * nb, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_blk_jlo, blk_jlo.data(), sizeof(int32_t) * nb, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_blk_ks, blk_ks.data(), sizeof(int32_t) * nb, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_grp_j0, grp_j0.data(), sizeof(int32_t) * ng, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(si->d_grp_kw, grp_kw.data(), sizeof(int32_t) * ng, cudaMemcpyHostToDevice, s);
+        // opt in to the shared memory of the widest block here, once, so that a call only launches
+        if (e == cudaSuccess && sizeof(double) * (size_t)kw_max * MM_DS > 48 * 1024)
+            e = cudaFuncSetAttribute(srcinterp_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * MM_KW_MAX * MM_DS));
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);   // the vectors die with this scope
     if (e != cudaSuccess) {
         gcamb_status st = cuda_fail(e, "gcamb_los_srcinterp_create");
@@ -222,9 +434,21 @@ gcamb_status gcamb_los_srcinterp_destroy(gcamb_los_srcinterp *si)
     if (e == cudaSuccess && cur != si->device) e = cudaSetDevice(si->device);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(si->d_h); cudaFree(si->d_ih); cudaFree(si->d_mult); cudaFree(si->d_inv_diag); cudaFree(si->d_seg); cudaFree(si->d_wgt);
+    cudaFree(si->d_blk_val); cudaFree(si->d_blk_off); cudaFree(si->d_blk_jlo); cudaFree(si->d_blk_ks); cudaFree(si->d_grp_j0); cudaFree(si->d_grp_kw);
     if (cur >= 0 && cur != si->device) cudaSetDevice(cur);
     delete si;
     if (e != cudaSuccess) return cuda_fail(e, "gcamb_los_srcinterp_destroy");
+    return GCAMB_OK;
+}
+
+gcamb_status gcamb_los_srcinterp_info(const gcamb_los_srcinterp *si, int32_t *n_kc, int32_t *n_k, int32_t *n_tau,
+                                      int32_t *band_columns)
+{
+    if (!si) { set_error("null handle"); return GCAMB_EINVAL; }
+    if (n_kc) *n_kc = si->n_kc;
+    if (n_k) *n_k = si->n_k;
+    if (n_tau) *n_tau = si->n_tau;
+    if (band_columns) *band_columns = si->n_iblk ? si->band_max : 0;
     return GCAMB_OK;
 }
 
@@ -238,6 +462,13 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *si, int32_t n_s
     GCAMB_CUDA(cudaGetDevice(&dev));
     if (dev != si->device) { set_error("handle belongs to device %d but device %d is current", si->device, dev); return GCAMB_EINVAL; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (si->n_iblk) {   // solve with the banded inverse on the FP64 tensor cores
+        dim3 gb((unsigned)((si->n_tau + MM_TAU - 1) / MM_TAU), (unsigned)si->n_grp, (unsigned)n_series);
+        srcinterp_mma_kernel<<<gb, 32 * MM_WARPS, sizeof(double) * (size_t)si->kw_max * MM_DS, s>>>(
+            d_S_coarse, d_work, si->d_ih, si->d_blk_val, si->d_blk_off, si->d_blk_jlo, si->d_blk_ks, si->d_grp_j0, si->d_grp_kw,
+            si->n_kc, si->n_tau, si->n_iblk);
+        GCAMB_CUDA(cudaGetLastError());
+    } else {
     // solve: 64 or 32 threads per block with the sweeps' intermediate in shared memory while it fits
     const size_t per_thread = sizeof(double) * (size_t)si->n_kc, tables = 4 * per_thread;
     const int threads = per_thread * 32 + tables <= 200 * 1024 ? 32 : 128;
@@ -251,9 +482,24 @@ gcamb_status gcamb_los_interp_sources(const gcamb_los_srcinterp *si, int32_t n_s
         srcinterp_solve_kernel<false><<<g1, threads, 0, s>>>(d_S_coarse, d_work, si->d_h, si->d_ih, si->d_mult, si->d_inv_diag, si->n_kc, si->n_tau);
     }
     GCAMB_CUDA(cudaGetLastError());
-    dim3 g2((unsigned)std::min((si->n_tau + 255) / 256, 16), (unsigned)((si->n_k + EVAL_ROWS - 1) / EVAL_ROWS), (unsigned)n_series);
-    srcinterp_eval_kernel<<<g2, 256, 0, s>>>(d_S_coarse, d_work, si->d_seg, si->d_wgt, d_S_fine, si->n_kc, si->n_k, si->n_tau);
-    GCAMB_CUDA(cudaGetLastError());
+    }
+    const bool vec2 = si->n_tau % 2 == 0 &&
+                      ((reinterpret_cast<uintptr_t>(d_S_coarse) | reinterpret_cast<uintptr_t>(d_work) | reinterpret_cast<uintptr_t>(d_S_fine)) & 15) == 0;
+    const int per_block = 256 * (vec2 ? 2 : 1);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)std::min((si->n_tau + per_block - 1) / per_block, 16), (unsigned)((si->n_k + EVAL_ROWS - 1) / EVAL_ROWS), (unsigned)n_series);
+    cfg.blockDim = dim3(256);
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const double *c_Sc = d_S_coarse, *c_M = d_work;
+    const int32_t *c_seg = si->d_seg;
+    const double4 *c_wgt = si->d_wgt;
+    GCAMB_CUDA(cudaLaunchKernelEx(&cfg, vec2 ? srcinterp_eval_kernel<2> : srcinterp_eval_kernel<1>, c_Sc, c_M, c_seg, c_wgt, d_S_fine,
+                                  si->n_kc, si->n_k, si->n_tau));
     return GCAMB_OK;
 }
 

@@ -25,7 +25,7 @@ EXPORTS = (
     "gcamb_los_spectra_batched", "gcamb_los_spectra_batched_info", "gcamb_los_cl_interp", "gcamb_los_last_error",
     "gcamb_los_tensor_work_bytes", "gcamb_los_transfer_tensor", "gcamb_los_cls_tensor",
     "gcamb_los_transfer_tensor_batched", "gcamb_los_cls_tensor_batched",
-    "gcamb_los_srcinterp_create", "gcamb_los_srcinterp_destroy", "gcamb_los_interp_sources",
+    "gcamb_los_srcinterp_create", "gcamb_los_srcinterp_destroy", "gcamb_los_srcinterp_info", "gcamb_los_interp_sources",
     "gcamb_los_interp_sources_noalloc",
 )
 # libgcamb_probe.so (include/gcamb_probe.h): bench.py's roofline probes, not part of the method
@@ -75,6 +75,7 @@ def load_library() -> ctypes.CDLL:
     lib.gcamb_los_cls_tensor_batched.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     lib.gcamb_los_srcinterp_create.argtypes = [ctypes.POINTER(_vp), _vp, _vp, _i32, _vp]
     lib.gcamb_los_srcinterp_destroy.argtypes = [_vp]
+    lib.gcamb_los_srcinterp_info.argtypes = [_vp] + [ctypes.POINTER(_i32)] * 4
     lib.gcamb_los_interp_sources.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp]
     lib.gcamb_los_interp_sources_noalloc.argtypes = [_vp, _i32, _vp, _vp, _vp]
     _lib = lib
@@ -301,6 +302,9 @@ class SourceInterp:
                                                          k_coarse.size, _stream()))
         self._h = handle
         self.n_kc, self.n_k, self.n_tau = int(k_coarse.size), plan.n_k, plan.n_tau
+        band = _i32()
+        _check(load_library().gcamb_los_srcinterp_info(self._h, None, None, None, ctypes.byref(band)))
+        self.band_columns = band.value          # 0: the solve runs as sequential sweeps
 
     def close(self) -> None:
         if getattr(self, "_h", None):

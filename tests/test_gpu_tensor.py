@@ -224,6 +224,47 @@ def test_interp_sources_against_the_oracle(los, shape):
     plan.close()
 
 
+@pytest.mark.parametrize("case", [
+    # (n_kc, n_k, n_tau, grid, banded): the solve runs with the banded inverse on the FP64 tensor cores, except for
+    # grids of fewer than 3 or more than 4096 coarse wavenumbers, which keep the sequential sweeps
+    (300, 900, 200, "log", True),
+    (9, 30, 33, "log", True),                 # one block of 8 rows + 1, odd n_tau: scalar evaluation kernel
+    (400, 300, 64, "alternating", True),      # spacings that jump by a factor 100 from one interval to the next
+    (4097, 200, 40, "log", False),
+    (2, 40, 32, "log", False),
+])
+def test_interp_sources_both_forms_of_the_solve(los, case):
+    n_kc, n_k, n_tau, grid, banded = case
+    if grid == "log":
+        kc = synth.k_grid(n_kc, 1e-5, 0.6)
+    else:
+        kc = 1e-4 + np.concatenate([[0.0], np.cumsum(np.where(np.arange(n_kc - 1) % 2 == 0, 1e-5, 1e-3))])
+    rng = np.random.default_rng(n_kc)
+    k = np.sort(np.concatenate([kc[[0, -1]], rng.uniform(kc[0], kc[-1], n_k - 2)]))
+    tau = np.linspace(100.0, 13900.0, n_tau)
+    plan = los.Plan(np.arange(2, 10, dtype=np.int32), k, tau, TAU0)
+    si = los.SourceInterp(plan, kc)
+    assert (si.band_columns > 0) == banded and si.band_columns <= 100
+    S_c = np.cos(30.0 * kc[:, None] * (1.0 + np.arange(n_tau)[None, :] / n_tau)) * np.exp(-(kc[:, None] / 0.3) ** 2)
+    S_c = S_c * (1.0 + 0.01 * rng.standard_normal((2,) + S_c.shape))
+    out = torch.full((2, n_k, n_tau), float("nan"), dtype=torch.float64, device="cuda")
+    si.gcamb_los_interp_sources(dev(S_c), out=out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    for s in range(2):
+        ref = oracle.interp_sources(kc, k, S_c[s], real="f80")
+        assert np.max(np.abs(got[s] - ref)) <= 1e-13 * np.max(np.abs(S_c[s]))
+    assert torch.equal(out, si.gcamb_los_interp_sources(dev(S_c)))          # deterministic
+    # an unaligned output buffer takes the scalar evaluation kernel: same values
+    if n_tau % 2 == 0:
+        buf = torch.empty(2 * n_k * n_tau + 1, dtype=torch.float64, device="cuda")
+        out2 = buf[1:].view(2, n_k, n_tau)
+        si.gcamb_los_interp_sources(dev(S_c), out=out2)
+        assert torch.equal(out2, out)
+    si.close()
+    plan.close()
+
+
 def test_interp_sources_feeds_the_transfer_kernel(los):
     """coarse sources -> InterpolateSources -> transfer -> C_l on the GPU against the same chain of the oracle."""
     cfg = synth.Config(9, "coarse-to-fine", 2, 300, 200, 1e-4, 0.05, 120, 60, False)
