@@ -25,6 +25,14 @@
 
 #include "los_internal.cuh"
 
+// -DGCAMB_DEBUG (GCAMB_DEBUG=1 python -m paper_2509_25110_b200.build --force): device asserts on the indices
+#ifdef GCAMB_DEBUG
+#include <cassert>
+#define GCAMB_ASSERT(c) assert(c)
+#else
+#define GCAMB_ASSERT(c) ((void)0)
+#endif
+
 struct gcamb_los_srcinterp {
     int32_t n_kc, n_k, n_tau, device;
     double *d_h;          // [n_kc]   h_i = kc_{i+1} - kc_i (last entry unused)
@@ -182,6 +190,7 @@ __global__ void __launch_bounds__(32 * MM_WARPS) srcinterp_mma_kernel(const doub
             for (int r = r0; r < r1; ++r) {
                 const int j = wj0 + r;
                 const double y2 = row(j + 1);
+                GCAMB_ASSERT(r >= 0 && r < Kw && Kw <= MM_KW_MAX && j >= 0 && j <= n_kc + 4 * MM_WARPS);
                 double d = 0.0;
                 if (tv && j >= 1 && j <= n_kc - 2) d = fma(y2 - y1, __ldg(ih + j), -((y1 - y0) * __ldg(ih + j - 1)));
                 dsm[r * MM_DS + lane] = d;
@@ -196,6 +205,7 @@ __global__ void __launch_bounds__(32 * MM_WARPS) srcinterp_mma_kernel(const doub
     const int ks = blk_ks[b], fr = lane >> 2, fc = lane & 3;
     const double *av = blk_val + blk_off[b] + lane;
     const double *dp = dsm + (blk_jlo[b] - wj0 + fc) * MM_DS + fr;
+    GCAMB_ASSERT(blk_jlo[b] >= wj0 && blk_jlo[b] - wj0 + 4 * ks <= Kw && blk_off[b] >= 0);   // every B fragment row lies in the block's window
     double D[MM_TAU / 8][2];
 #pragma unroll
     for (int nt = 0; nt < MM_TAU / 8; ++nt) D[nt][0] = D[nt][1] = 0.0;
@@ -212,6 +222,7 @@ __global__ void __launch_bounds__(32 * MM_WARPS) srcinterp_mma_kernel(const doub
 #pragma unroll
         for (int nt = 0; nt < MM_TAU / 8; ++nt) {
             const int t = tau0 + 8 * nt + 2 * fc;
+            GCAMB_ASSERT(row >= 0 && row < n_kc && t >= 0);
             if (t < n_tau) m[t] = D[nt][0];
             if (t + 1 < n_tau) m[t + 1] = D[nt][1];
         }
@@ -252,6 +263,7 @@ __global__ void __launch_bounds__(256) srcinterp_eval_kernel(const double *__res
         for (int u = 0; u < EVAL_ROWS; ++u) {
             if (j0 + u < j_end) {
                 const size_t c = cbase + (size_t)sg[u] * n_tau + t, f = ((size_t)blockIdx.z * n_k + j0 + u) * n_tau + t;
+                GCAMB_ASSERT(sg[u] >= 0 && sg[u] + 1 < n_kc && t + VEC <= n_tau && j0 + u < n_k);
                 if (VEC == 2) {
                     const double2 ya = *reinterpret_cast<const double2 *>(S_c + c), yb = *reinterpret_cast<const double2 *>(S_c + c + n_tau);
                     const double2 ma = *reinterpret_cast<const double2 *>(M + c), mb = *reinterpret_cast<const double2 *>(M + c + n_tau);
