@@ -56,6 +56,7 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_korder); cudaFree(p->d_l_list); cudaFree(p->d_kz); cudaFree(p->d_tile_mask);
     cudaFree(p->d_bin_start); cudaFree(p->d_bin_items); cudaFree(p->d_fused_scratch);
     cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg); cudaFree(p->d_l_user);
+    cudaFree(p->d_sp_ainv); cudaFree(p->d_sp_aoff); cudaFree(p->d_sp_alo); cudaFree(p->d_sp_acnt);
     cudaFree(p->d_cth); cudaFree(p->d_s2); cudaFree(p->d_ib2); cudaFree(p->d_coef); cudaFree(p->d_l_end);
     cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_cE); cudaFree(p->d_t_cB);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);

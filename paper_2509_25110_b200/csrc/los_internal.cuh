@@ -66,6 +66,8 @@ struct gcamb_los_plan {
     double *d_sp_mult;       // [n_l] forward-elimination multipliers
     double *d_sp_inv_diag;   // [n_l] reciprocals of the eliminated diagonal
     int32_t *d_sp_seg;       // [l_max - l_min + 1] knot interval of every integer l
+    double *d_sp_ainv;       // banded inverse of the spline matrix, packed rows (interp.cu); NULL: the sequential sweeps are used
+    int32_t *d_sp_aoff, *d_sp_alo, *d_sp_acnt;   // [n_l] offset, first column and number of columns of row i
     int32_t *d_l_user;       // [n_l_out] the caller's l list (knots of the spline)
 
     // open-universe plans: d_chi holds chi_i = (tau0 - tau_i)/r_c; d_inv is not allocated

@@ -57,7 +57,9 @@ def interp_err(C_gpu, C_ref):
     [2, 3, 4, 5, 6],                               # every l listed: nothing to interpolate
     [5, 6, 8, 9, 40, 41, 300, 1000, 1001, 2500],   # neighbouring knots next to long gaps
     list(camb_like_list(2, 2500)),
-    list(range(2, 3000, 3)),                       # 1000 knots: the sequential sweeps are long
+    list(range(2, 3000, 3)),                       # 1000 knots
+    list(range(2, 6500, 3)),                       # 2166 knots > 2048: the sequential sweeps by one thread
+    [2, 3, 50, 51, 52, 400, 2000, 2001, 2002, 2003, 5000],   # spacings that jump by three orders of magnitude
 ])
 def test_spline_kernel_on_smooth_spectra_against_the_oracle(los, l_list):
     l_list = np.asarray(l_list, dtype=np.int32)
