@@ -479,7 +479,7 @@ def time_steps(step_fns, steps: int, warmup: int, flush):
 
 
 def run_next(args) -> None:
-    """One JSON line for a SURVEY 8(f) row: --workload sparse | tensor | open | srcinterp (single GPU)."""
+    """One JSON line for a SURVEY 8(f) row: --workload sparse | tensor | open | srcinterp | emulator (single GPU)."""
     import torch
 
     import oracle
@@ -551,6 +551,33 @@ def run_next(args) -> None:
         algorithmic = "10 flop per executed (l,k,tau): A_l coth, R_l f_{l+1}, recurrence, 2 accumulates"
         ref = lambda sl: oracle.transfer_open(l_list, k[sl], tau, tau0, K, S[0][sl], S[1][sl], real="f64", nthreads=cores)
         get_rows = lambda rows: D[:, :, rows]
+    elif w == "emulator":  # NEXT-1 + NEXT-2: the batch of config 3 on CAMB's default l sampling, fused kernel + spline to every l
+        cfg3 = synth.CONFIGS[3]
+        B = cfg3.n_batch
+        k, l_list = cfg3.k(), camb_like_l_list(cfg3.l_min, cfg3.l_max)
+        S0 = synth.sources(cfg3, 0)
+        dT = torch.empty((B, cfg3.n_k, cfg3.n_tau), dtype=torch.float64, device=dev)
+        dE = torch.empty_like(dT)
+        hP = np.stack([synth.primordial_power(cfg3, c) for c in range(B)])
+        for c in range(B):
+            Sc_ = S0 if c == 0 else synth.sources(cfg3, c)
+            dT[c].copy_(torch.from_numpy(Sc_[0])); dE[c].copy_(torch.from_numpy(Sc_[1]))
+        dP = to_dev(hP)
+        plan = los.Plan(l_list, k, tau, tau0)
+        info = plan.gcamb_los_spectra_batched_info(B)
+        C = torch.empty((B, 3, plan.n_l), dtype=torch.float64, device=dev)
+        C_all = torch.empty((B, 3, plan.n_l_all), dtype=torch.float64, device=dev)
+        fns = [lambda: plan.gcamb_los_spectra_batched(dT, dE, None, dP, out=C), lambda: plan.gcamb_los_cl_interp(C, out=C_all)]
+        names = ["spectra_batched_ms", "cl_interp_ms"]
+        # algorithmic work: coefficient + recurrence once per executed (l, k, tau) for a block of 8 cosmologies, two
+        # accumulates per cosmology on the LISTED l only; the listed share of the executed terms, exactly
+        x = k[:, None] * (tau0 - tau)[None, :]
+        L = np.minimum(np.ceil(x + 18.2 * np.cbrt(x) + 8.0), cfg3.l_max)          # reading R16
+        n_exec = np.maximum(L - cfg3.l_min + 1, 0.0)
+        n_listed = np.searchsorted(l_list, L, side="right").astype(np.float64)
+        f_listed = float(n_listed.sum() / n_exec.sum())
+        workload = (f"config 3 batch ({B} cosmologies, config-1 grids) on a CAMB-like list of {l_list.size} of {plan.n_l_all} "
+                    f"multipoles: gcamb_los_spectra_batched ({'fused kernel' if info['fused'] else 'two kernels'}) + spline to every l")
     else:                  # srcinterp, NEXT-3: 300 evolved wavenumbers -> the 3000 of config 1, T and E
         k, kc = cfg.k(), synth.k_grid(300, cfg.k_lo, cfg.k_hi)
         coarse = synth.Config(9, "coarse", cfg.l_min, cfg.l_max, 300, cfg.k_lo, cfg.k_hi, cfg.n_tau_uniform, cfg.n_tau_log, False)
@@ -567,7 +594,28 @@ def run_next(args) -> None:
     clocks = sampler.stop()
     t_step = sum(times) * 1e-3
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
-    if w == "srcinterp":
+    if w == "emulator":
+        executed = plan.executed_terms
+        flop = 2.0 * (2.0 / 8.0 + 2.0 * f_listed)
+        achieved = executed * B * flop / (times[0] * 1e-3) / 1e12
+        value, unit, metric = plan.n_l_all * plan.n_k * plan.n_tau * B / t_step, UNIT, "LOS (l,k,tau) terms/s"
+        roof = {"bound": "alu", "kernel": "fused_kernel", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": achieved / peak_tf, "traffic": None,
+                "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md section 7)",
+                "algorithmic": (f"{flop:.3f} flop per executed (l,k,tau,cosmology): coefficient + recurrence shared by 8 cosmologies, 2 "
+                                f"accumulates on the {100 * f_listed:.1f} % of the executed terms whose l is listed; x {executed} executed "
+                                f"terms x {B} cosmologies; the kernel accumulates whole l-tiles of 8 (every tile that holds a listed l)")}
+        extra = {"executed_terms_per_s": executed * B / t_step, "spectra_per_s": B / t_step, "fused": bool(info["fused"])}
+        t0 = time.perf_counter()
+        D_ref = oracle.transfer(l_list, k, tau, tau0, S0[0], S0[1], real="f64", nthreads=cores)
+        C_ref = oracle.cl_interp(l_list, oracle.cls(k, D_ref, hP[0], real="f64"), real="f64")
+        dt = time.perf_counter() - t0
+        got = C_all[0].cpu().numpy()
+        err = float(max(np.max(np.abs(got[:2] / C_ref[:2] - 1.0)),
+                        np.max(np.abs(got[2] - C_ref[2]) / np.sqrt(C_ref[2] ** 2 + C_ref[0] * C_ref[1]))))
+        cpu = {"value": 1.0 / dt, "unit": "spectra/s", "cores": cores, "kind": "oracle",
+               "sample": f"cosmology 0 in full (sparse transfer + cls + spline), fp64 oracle build, {dt:.1f} s", "cl_err_on_sample": err}
+    elif w == "srcinterp":
         # algorithmic bytes: coarse sources read once, second derivatives written and read once, fine sources written
         n_c, n_f = int(dSc.numel()), int(out.numel())
         bytes_alg = 8 * (3 * n_c + n_f)
@@ -629,7 +677,7 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=1, choices=range(len(synth.CONFIGS)))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="config", choices=["config", "sparse", "tensor", "open", "srcinterp"],
+    ap.add_argument("--workload", default="config", choices=["config", "sparse", "tensor", "open", "srcinterp", "emulator"],
                     help="config: BASELINE.json's configs (--config); the others: SURVEY 8(f) rows, one GPU")
     args = ap.parse_args()
     if args.workload != "config":

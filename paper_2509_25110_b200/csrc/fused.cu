@@ -44,6 +44,7 @@ struct FusedParams {
     const double *k, *chi, *w, *pref, *inv_x, *dlnk;
     const double2 *start;
     const int32_t *tile, *l_index, *bin_start, *bin_items;
+    const uint32_t *tile_mask;   // sparse l lists: bit t % 32 of word t / 32 = tile t holds a listed l
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_bins, l_contig;
 };
 
@@ -63,6 +64,31 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b)
                  : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
 
+// The recurrence alone on one l-tile for the first NA slots of a thread (tiles without a listed l of the SPARSE
+// kernel): NA chains interleaved (l outer, slot inner), compensated coefficient as in the MMA path.
+template <int NA, int T>
+__device__ __forceinline__ void fused_walk(double tl0, const double *my_ix, const double *my_ixlo, double (&fa)[T], double (&fb)[T])
+{
+    static_assert(T <= 10, "the dispatch on the number of started slots is written out for T <= 10");
+    double ixr[NA], er[NA];
+#pragma unroll
+    for (int j = 0; j < NA; ++j) {
+        ixr[j] = my_ix[j * F_THREADS];
+        er[j] = tl0 * my_ixlo[j * F_THREADS];
+    }
+#pragma unroll
+    for (int s = 0; s < F_V; ++s) {
+        const double tl = tl0 - 2.0 * s;
+#pragma unroll
+        for (int j = 0; j < NA; ++j) {
+            const double c = fma(tl, ixr[j], er[j]);
+            const double fn = fma(c, fb[j], -fa[j]);
+            fa[j] = fb[j];
+            fb[j] = fn;
+        }
+    }
+}
+
 template <int NB, int T> constexpr size_t fused_smem_bytes()
 {
     constexpr int P = F_V * 8 * NB;
@@ -74,7 +100,12 @@ template <int NB, int T> constexpr size_t fused_smem_bytes()
 }
 
 // NB = 8-column blocks of the contraction: BC = 4 NB cosmologies x (T, E).  T = points per thread.
-template <int NB, int T>
+// SPARSE (l lists with l-tiles that hold no listed l: CAMB's default l sampling): such a tile is
+// walked by the recurrence alone (16 FP64 instructions per started slot instead of those plus 16 MMAs), nothing of
+// it enters the ring, and its rows are skipped by the flush (the groups of tiles keep their places in the ring:
+// taking the groups without a listed l out of the barrier protocol measured 16.0 against 13.3 ms, registers).
+// A kernel of its own: the dense kernel is unchanged.
+template <int NB, int T, bool SPARSE>
 __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p)
 {
     constexpr int V = F_V, W = F_W, G = F_G, RD = F_RD, LAG = F_LAG, JS = F_JS;
@@ -217,6 +248,7 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
     int next_slot = GCAMB_UNI(slot_win[0]);
     int inj = 0, inj_from = next_slot;
     int buf = 0;
+    unsigned mask_word = 0;
     double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);
     const int n_groups = (n_walk + G - 1) / G;
     int t = t_begin;
@@ -242,7 +274,21 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
                 inj_from = inj < T ? GCAMB_UNI(slot_win[2 * inj]) : NEVER;
             }
             double2 *rb = reinterpret_cast<double2 *>(ring + ((size_t)((n % RD) * G + g) * W + warp) * P);
-            if (na > 0) {
+            bool listed = true;
+            if constexpr (SPARSE) {
+                if ((t & 31) == 0 || t == t_begin) mask_word = GCAMB_UNI(p.tile_mask[t >> 5]);
+                listed = (mask_word >> (t & 31)) & 1u;
+            }
+            if (SPARSE && !listed) {
+                // a2 alone for the started slots: no tile of j_l, no MMA, no ring entry.  One body per number of
+                // started slots (a run-time bound inside the unrolled loops turns into selects on every state register)
+#define GCAMB_FW(n) case n: if constexpr (T >= n) fused_walk<n, T>(tl0, my_ix, my_ixlo, fa, fb); break;
+                switch (na) {
+                    GCAMB_FW(1) GCAMB_FW(2) GCAMB_FW(3) GCAMB_FW(4) GCAMB_FW(5)
+                    GCAMB_FW(6) GCAMB_FW(7) GCAMB_FW(8) GCAMB_FW(9) GCAMB_FW(10)
+                }
+#undef GCAMB_FW
+            } else if (na > 0) {
                 double D[2][NB][2];   // even / odd MMAs accumulate apart: 2 NB independent chains
 #pragma unroll
                 for (int h = 0; h < 2; ++h)
@@ -327,20 +373,26 @@ __global__ void __launch_bounds__(256) fused_finish_kernel(const double *__restr
     Cl[((size_t)b * 3 + spec) * n_l + li] = 4.0 * 3.14159265358979323846 * s;
 }
 
-template <int NB, int T>
-gcamb_status launch_one(const FusedParams &prm, int n_cblk, int device, cudaStream_t stream)
+template <int NB, int T, bool SPARSE>
+gcamb_status launch_sp(const FusedParams &prm, int n_cblk, int device, cudaStream_t stream)
 {
     constexpr size_t smem = fused_smem_bytes<NB, T>();
     static_assert(smem <= 227 * 1024, "shared memory of the fused kernel");
     static std::atomic<unsigned long long> attr_done;
     const unsigned long long dev_bit = 1ull << (device & 63);
     if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
-        GCAMB_CUDA(cudaFuncSetAttribute(fused_kernel<NB, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GCAMB_CUDA(cudaFuncSetAttribute(fused_kernel<NB, T, SPARSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done.fetch_or(dev_bit, std::memory_order_release);
     }
-    fused_kernel<NB, T><<<dim3((unsigned)prm.n_bins, (unsigned)n_cblk), F_THREADS, smem, stream>>>(prm);
+    fused_kernel<NB, T, SPARSE><<<dim3((unsigned)prm.n_bins, (unsigned)n_cblk), F_THREADS, smem, stream>>>(prm);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
+}
+
+template <int NB, int T>
+gcamb_status launch_one(const FusedParams &prm, int n_cblk, int device, cudaStream_t stream)
+{
+    return prm.tile_mask ? launch_sp<NB, T, true>(prm, n_cblk, device, stream) : launch_sp<NB, T, false>(prm, n_cblk, device, stream);
 }
 
 }  // namespace
@@ -371,7 +423,7 @@ gcamb_status launch_fused(const gcamb_los_plan *p, int n_batch, const double *S_
     prm.S_T = S_T; prm.S_E = S_E; prm.P_R = P_R; prm.Cpart = scratch;
     prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref; prm.inv_x = p->d_inv; prm.dlnk = p->d_dlnk;
     prm.start = p->d_start; prm.tile = p->d_tile; prm.l_index = p->d_l_index;
-    prm.bin_start = p->d_bin_start; prm.bin_items = p->d_bin_items;
+    prm.bin_start = p->d_bin_start; prm.bin_items = p->d_bin_items; prm.tile_mask = p->d_tile_mask;
     prm.n_k = p->n_k; prm.n_tau = p->n_tau; prm.n_l = p->n_l; prm.l_min = p->l_min; prm.l_max = p->l_max;
     prm.n_tiles = p->n_tiles; prm.n_batch = n_batch; prm.n_bins = p->n_bins;
     prm.l_contig = p->n_l == p->l_max - p->l_min + 1;
