@@ -265,6 +265,38 @@ def test_interp_sources_both_forms_of_the_solve(los, case):
     plan.close()
 
 
+def test_interp_sources_captures_into_a_cuda_graph(los):
+    """The call only enqueues its two kernels (the second one as a programmatic dependent launch of the first), so
+    it can be captured once and replayed on new coarse sources, with caller scratch or with the static scratch."""
+    kc = synth.k_grid(50, 1e-5, 0.6)
+    k = synth.k_grid(333, 1e-5, 0.6)
+    tau = np.linspace(100.0, 13900.0, 96)
+    plan = los.Plan(np.arange(2, 10, dtype=np.int32), k, tau, TAU0)
+    si = los.SourceInterp(plan, kc)
+    rng = np.random.default_rng(3)
+    d_S = dev(rng.standard_normal((2, 50, 96)))
+    work = torch.empty_like(d_S)
+    out = torch.empty(2, 333, 96, dtype=torch.float64, device="cuda")
+    out_static = torch.empty_like(out)
+    si.gcamb_los_interp_sources(d_S, out=out, work=work)
+    si.gcamb_los_interp_sources_noalloc(d_S, out_static)           # first call on the device: outside the capture
+    torch.cuda.synchronize()
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            si.gcamb_los_interp_sources(d_S, out=out, work=work)
+            si.gcamb_los_interp_sources_noalloc(d_S, out_static)
+    for _ in range(2):
+        d_S.copy_(dev(rng.standard_normal((2, 50, 96))))
+        out.fill_(float("nan")); out_static.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        want = si.gcamb_los_interp_sources(d_S)
+        assert torch.equal(out, want) and torch.equal(out_static, want)
+    si.close()
+    plan.close()
+
+
 def test_interp_sources_feeds_the_transfer_kernel(los):
     """coarse sources -> InterpolateSources -> transfer -> C_l on the GPU against the same chain of the oracle."""
     cfg = synth.Config(9, "coarse-to-fine", 2, 300, 200, 1e-4, 0.05, 120, 60, False)
