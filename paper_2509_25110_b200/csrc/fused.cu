@@ -229,8 +229,14 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
     }
 
     // flush of group m: warps summed in index order, Delta^E prefactor, Eq. 1 products into the partial spectra
-    auto flush_group = [&](int m) {
+    // has: some tile of the group holds a listed l (always, unless SPARSE).  A group without one leaves nothing in
+    // the ring: its flush neither waits for the other warps nor reads, it only hands the stage back
+    auto flush_group = [&](int m, bool has) {
         const int stage = m % RD;
+        if (SPARSE && !has) {
+            if (lane == 0) mbar_arrive(bar_empty + 8 * stage);
+            return;
+        }
         const int gcount = min(G, n_walk - m * G);
         // this thread's (l, cosmology) and its three partial spectra: the loads (L2 round trips: the
         // source view showed 8 % of the warp time waiting for them behind the ring sums) are issued
@@ -270,7 +276,7 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
     int next_slot = GCAMB_UNI(slot_win[0]);
     int inj = 0, inj_from = next_slot;
     int buf = 0;
-    unsigned mask_word = 0;
+    unsigned mask_word = 0, any_hist = 0;   // SPARSE; bit i of any_hist: group n - i holds a listed l
     double tl0 = (double)(2 * (p.l_max - t_begin * V) + 1);
     const int n_groups = (n_walk + G - 1) / G;
     int t = t_begin;
@@ -300,6 +306,7 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
             if constexpr (SPARSE) {
                 if ((t & 31) == 0 || t == t_begin) mask_word = GCAMB_UNI(p.tile_mask[t >> 5]);
                 listed = (mask_word >> (t & 31)) & 1u;
+                any_hist |= (unsigned)listed;
             }
             if (SPARSE && !listed) {
                 // a2 alone for the started slots: no tile of j_l, no MMA, no ring entry.  One body per number of
@@ -370,7 +377,8 @@ __global__ void __launch_bounds__(F_THREADS, 1) fused_kernel(const FusedParams p
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_full + 8 * (n % RD));
       }
-      if (n >= LAG) flush_group(n - LAG);
+      if (n >= LAG) flush_group(n - LAG, (any_hist >> LAG) & 1u);
+      any_hist <<= 1;
     }
 #undef GCAMB_UNI
   }   // k rows of this bin
