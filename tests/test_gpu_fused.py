@@ -109,6 +109,39 @@ def test_fused_with_a_sparse_l_list(los):
     plan.close()
 
 
+@pytest.mark.parametrize("shape", [
+    # (l_max, n_k, n_tau_uniform, n_tau_log, batch): the recurrence-only tiles with 1..10 slots per thread
+    (900, 20, 600, 600, 8),        # T = 5, blocks of 8 cosmologies
+    (700, 14, 250, 133, 9),        # T = 2, ragged batch, odd n_tau
+    (600, 10, 900, 700, 5),        # n_tau = 1600 > 1280: blocks of 4, T = 8
+    (500, 8, 1300, 1260, 4),       # n_tau = 2560: T = 10
+])
+def test_fused_sparse_lists_against_the_two_kernel_path_and_the_oracle(los, shape):
+    l_max, n_k, n_u, n_log, B = shape
+    cfg = synth.Config(9, "fused-sparse-shapes", 2, l_max, n_k, 1e-4, 0.3, n_u, n_log, False, n_batch=B)
+    rng = np.random.default_rng(l_max)
+    l_list = np.unique(np.concatenate([np.arange(2, 12), rng.choice(np.arange(12, l_max), size=25, replace=False),
+                                       [l_max]])).astype(np.int32)
+    hS, hP = batch_inputs(cfg)
+    plan = los.Plan(l_list, cfg.k(), cfg.tau(), cfg.tau0)
+    assert plan.gcamb_los_spectra_batched_info(B)["fused"]
+    d_T, d_E, d_P = dev(hS[0]), dev(hS[1]), dev(hP)
+    C = torch.full((B, 3, l_list.size), float("nan"), dtype=torch.float64, device="cuda")
+    plan.gcamb_los_spectra_batched(d_T, d_E, None, d_P, out=C)
+    torch.cuda.synchronize()
+    assert torch.equal(C, plan.gcamb_los_spectra_batched(d_T, d_E, None, d_P))        # deterministic
+    C_two = plan.gcamb_los_cls_batched(plan.gcamb_los_transfer_batched(d_T, d_E), d_P).cpu().numpy()
+    C = C.cpu().numpy()
+    assert np.all(np.isfinite(C))
+    e_auto, e_te = cl_err(C, C_two)                                                    # same sums in another order
+    assert e_auto <= 1e-11 and e_te <= 1e-11
+    c = B - 1
+    D_ref = oracle.transfer(l_list, cfg.k(), cfg.tau(), cfg.tau0, hS[0][c], hS[1][c], real="f80")
+    e_auto, e_te = cl_err(C[c], oracle.cls(cfg.k(), D_ref, hP[c], real="f80"))
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
 def test_emulator_step_captures_into_a_cuda_graph(los):
     """SURVEY 8(f) NEXT-1, second half: the whole batched step (fused kernel, finish kernel, spline to every l)
     only enqueues work on the caller's stream, so an emulator loop captures it once and replays it on new
