@@ -531,10 +531,11 @@ def run_next(args) -> None:
         work = torch.empty(plan.gcamb_los_tensor_work_bytes() // 8, dtype=torch.float64, device=dev)
         fns = [lambda: plan.gcamb_los_transfer_tensor(*dS, out=D, work=work), lambda: plan.gcamb_los_cls_tensor(D, dP, out=C)]
         names = ["transfer_ms", "cls_ms"]
-        flop_per_term, units = 2 * 8, plan.n_l * plan.n_k * plan.n_tau
+        flop_per_term, units = 2 * 6, plan.n_l * plan.n_k * plan.n_tau
         workload = "tensor modes: l=2..1500, n_k=1000 log in [1e-5, 3000/tau0], config-1 tau grid (1200), sources T,E,B (reading R27)"
-        algorithmic = ("16 flop per executed (l,k,tau): coefficient + recurrence + the 6 plain sums of the T, E, B kernels; "
-                       "the path executes 20 (two runs of the three-source kernels)")
+        algorithmic = ("12 flop per executed (l,k,tau): coefficient + recurrence + the 4 plain sums the T, E, B kernels reduce to "
+                       "(the sums with one power of 1/x follow from those without through j_l/x = (j_{l-1} + j_{l+1})/(2l+1)); "
+                       "the path executes 16 (two runs of the two-source kernels)")
         ref = lambda sl: oracle.transfer_tensor(l_list, k[sl], tau, tau0, S[0][sl], S[1][sl], S[2][sl], real="f64", nthreads=cores)
         get_rows = lambda rows: D[:, :, rows]
     elif w == "open":      # NEXT-4: config-1 grids in an open universe, r_c = 14000 Mpc

@@ -67,7 +67,7 @@ enum { GCAMB_SRC_T = 1, GCAMB_SRC_E = 2, GCAMB_SRC_PHI = 4, GCAMB_SRC_TENSOR = 8
  *                        the batched calls: one thread block per k row and cosmology)
  *   tau     HOST [n_tau] strictly increasing, < tau0, finite; n_tau >= 2
  *   src_mask             GCAMB_SRC_T|GCAMB_SRC_E, GCAMB_SRC_T|GCAMB_SRC_E|GCAMB_SRC_PHI, or GCAMB_SRC_TENSOR
- *                        (tensor plan: l <= 65534, three sources, four spectra; only the *_tensor calls,
+ *                        (tensor plan: l <= 65533, three sources, four spectra; only the *_tensor calls,
  *                        gcamb_los_cl_interp and gcamb_los_srcinterp_create accept it)
  *   cuda_stream          stream the precompute kernels run on; the call synchronises it.
  * On success *out owns device memory on the CURRENT device; free with gcamb_los_plan_destroy.
@@ -198,10 +198,11 @@ gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, co
  *   Delta^{B,t}_l(k) = sum_i w_i S_B(k,tau_i) [ 2 j_l' + 4 j_l/x ](x_i)
  *   C_l^{XY,t}       = 4 pi sum_j dlnk_j P_t(k_j) Delta^{X,t}_l(k_j) Delta^{Y,t}_l(k_j),  XY = TT, EE, BB, TE
  * (Eq. 1 with the tensor primordial spectrum; convention constants of the tensor normalisation belong to
- * P_t).  `plan` must have been created with src_mask = GCAMB_SRC_TENSOR.  The transfer call runs the
- * three-source transfer kernels twice on the union of {l} and {l + 1} (the E and B kernels are
- * combinations of plain j_l and j_{l+1} sums with l-dependent coefficients) plus two small kernels; it
- * needs caller-owned scratch of gcamb_los_tensor_work_bytes() bytes PER COSMOLOGY.
+ * P_t).  `plan` must have been created with src_mask = GCAMB_SRC_TENSOR (2 <= l <= 65533).  The transfer call
+ * runs the two-source transfer kernels twice on the union of {l - 1, l, l + 1, l + 2} (the T, E and B kernels
+ * are combinations, with l-dependent coefficients, of four plain j_l sums at neighbouring multipoles, through
+ * j_l' = (l/x) j_l - j_{l+1} and j_l/x = (j_{l-1} + j_{l+1})/(2l+1)) plus two small kernels; it needs
+ * caller-owned scratch of gcamb_los_tensor_work_bytes() bytes PER COSMOLOGY.
  *   d_S_T, d_S_E, d_S_B DEVICE [n_k][n_tau];  d_Delta DEVICE [3][n_l][n_k], order T, E, B;
  *   d_work DEVICE scratch;  d_P_t DEVICE [n_k];  d_Cl DEVICE [4][n_l], order TT, EE, BB, TE.
  * The *_batched forms take n_batch cosmologies on one plan (a5; emulator use-case PAPER.md:24, 248), every

@@ -1,5 +1,6 @@
 // api.cu -- the extern "C" boundary (include/gcamb_los.h): validation, host-side plan tables,
 // launches.  No step of the hot path runs on the host.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -58,7 +59,8 @@ static void free_plan(gcamb_los_plan *p)
     cudaFree(p->d_sp_mult); cudaFree(p->d_sp_inv_diag); cudaFree(p->d_sp_seg); cudaFree(p->d_l_user);
     cudaFree(p->d_sp_ainv); cudaFree(p->d_sp_aoff); cudaFree(p->d_sp_alo); cudaFree(p->d_sp_acnt);
     cudaFree(p->d_cth); cudaFree(p->d_s2); cudaFree(p->d_ib2); cudaFree(p->d_coef); cudaFree(p->d_l_end);
-    cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_cE); cudaFree(p->d_t_cB);
+    cudaFree(p->d_t_posm); cudaFree(p->d_t_pos0); cudaFree(p->d_t_pos1); cudaFree(p->d_t_pos2);
+    cudaFree(p->d_t_cE); cudaFree(p->d_t_cB); cudaFree(p->d_t_c3);
     for (int q = 0; q < 3; ++q) cudaFree(p->d_hS[q]);
     cudaFree(p->d_hP); cudaFree(p->d_hDelta); cudaFree(p->d_hCl);
     if (p->h_streams_ready) {
@@ -126,22 +128,26 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
         set_error("src_mask must be T|E, T|E|PHI or TENSOR");
         return GCAMB_EINVAL;
     }
-    const int l_top = tensor ? 65534 : 65535;   // a tensor plan also walks l + 1
+    const int l_top = tensor ? 65533 : 65535;   // a tensor plan also walks l + 1 and l + 2
     for (int i = 0; i < n_l; ++i) {
         if (l_list[i] < 2 || l_list[i] > l_top) { set_error("l_list[%d] = %d outside [2, %d]", i, l_list[i], l_top); return GCAMB_EINVAL; }
         if (i && l_list[i] <= l_list[i - 1]) { set_error("l_list not strictly increasing at %d", i); return GCAMB_EINVAL; }
     }
-    // Tensor plans (tensor.cu): the E and B kernels need j_{l+1} next to j_l, so the kernels run on the
-    // union of {l} and {l + 1}; the caller's list and the positions of l and l + 1 in the union are kept.
+    // Tensor plans (tensor.cu): every tensor transfer function is a combination of PLAIN sums at l - 1 .. l + 2, so
+    // the kernels run on the union of those lists (l - 1 may be 1); the caller's list and the rows of l - 1 .. l + 2
+    // in the union are kept.
     const int32_t *user_list = l_list;
     const int32_t n_user = n_l;
-    std::vector<int32_t> ext, pos0, pos1;
+    std::vector<int32_t> ext, posm, pos0, pos1, pos2;
     if (tensor) {
+        for (int i = 0; i < n_l; ++i)
+            for (int d = -1; d <= 2; ++d) ext.push_back(l_list[i] + d);
+        std::sort(ext.begin(), ext.end());
+        ext.erase(std::unique(ext.begin(), ext.end()), ext.end());
+        auto row_of = [&](int l) { return (int32_t)(std::lower_bound(ext.begin(), ext.end(), l) - ext.begin()); };
         for (int i = 0; i < n_l; ++i) {
-            if (ext.empty() || ext.back() != l_list[i]) ext.push_back(l_list[i]);
-            pos0.push_back((int32_t)ext.size() - 1);
-            ext.push_back(l_list[i] + 1);
-            pos1.push_back((int32_t)ext.size() - 1);
+            posm.push_back(row_of(l_list[i] - 1)); pos0.push_back(row_of(l_list[i]));
+            pos1.push_back(row_of(l_list[i] + 1)); pos2.push_back(row_of(l_list[i] + 2));
         }
         l_list = ext.data();
         n_l = (int32_t)ext.size();
@@ -166,6 +172,8 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     p->r_c = curved ? 1.0 / std::sqrt(std::fabs(curv_K)) : 0.0;
     p->src_mask = src_mask;
     p->n_src = (tensor || (src_mask & GCAMB_SRC_PHI)) ? 3 : 2;
+    p->n_src_walk = tensor ? 2 : p->n_src;
+    p->l_user_first = user_list[0]; p->l_user_last = user_list[n_user - 1];
     p->n_spec = p->n_src + 1;
     p->l_min = l_list[0]; p->l_max = l_list[n_l - 1];
     p->tau0 = tau0;
@@ -176,7 +184,7 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     cudaError_t e = cudaGetDevice(&p->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
     if (e != cudaSuccess) { gcamb_status st = cuda_fail(e, "device query"); free_plan(p); return st; }
-    p->shape = choose_shape(n_tau, p->n_src, n_k, p->n_sm);
+    p->shape = choose_shape(n_tau, p->n_src_walk, n_k, p->n_sm);
     p->n_tiles = (p->l_max - p->l_min) / p->shape.V + 1;
 
     // IntegrationVars_init: the O(N) tables, on the host in fp64
@@ -224,17 +232,21 @@ static gcamb_status create_plan(gcamb_los_plan **out, const int32_t *l_list, int
     if (e == cudaSuccess) e = upload(&p->d_l_list, std::vector<int32_t>(l_list, l_list + n_l), stream);
     if (e == cudaSuccess) e = upload(&p->d_l_user, std::vector<int32_t>(user_list, user_list + n_user), stream);
     if (tensor) {
-        // combination coefficients of tensor.cu: (l+1)(l+2)/sqrt((l+2)(l+1)l(l-1)) and 2(l+2)
-        std::vector<double> cE(n_user), cB(n_user);
+        // combination coefficients of tensor.cu
+        std::vector<double> cE(n_user), cB(n_user), c3(n_user);
         for (int i = 0; i < n_user; ++i) {
             const double l = user_list[i];
             cE[i] = (l + 1.0) * (l + 2.0) / std::sqrt((l + 2.0) * (l + 1.0) * l * (l - 1.0));
-            cB[i] = 2.0 * (l + 2.0);
+            cB[i] = 2.0 * (l + 2.0) / (2.0 * l + 1.0);
+            c3[i] = 1.0 / (2.0 * l + 3.0);
         }
+        if (e == cudaSuccess) e = upload(&p->d_t_posm, posm, stream);
         if (e == cudaSuccess) e = upload(&p->d_t_pos0, pos0, stream);
         if (e == cudaSuccess) e = upload(&p->d_t_pos1, pos1, stream);
+        if (e == cudaSuccess) e = upload(&p->d_t_pos2, pos2, stream);
         if (e == cudaSuccess) e = upload(&p->d_t_cE, cE, stream);
         if (e == cudaSuccess) e = upload(&p->d_t_cB, cB, stream);
+        if (e == cudaSuccess) e = upload(&p->d_t_c3, c3, stream);
     }
     {   // sparse l lists: which tiles hold a listed l (NULL table = all of them)
         std::vector<uint32_t> mask((p->n_tiles + 31) / 32, 0u);

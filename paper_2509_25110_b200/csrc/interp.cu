@@ -268,7 +268,7 @@ gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double
     if (smem > 48 * 1024)
         GCAMB_CUDA(cudaFuncSetAttribute(cl_interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long series = (long long)n_batch * p->n_spec;
-    const int n_all = p->l_max - p->tensor - p->l_min + 1;
+    const int n_all = p->l_user_last - p->l_user_first + 1;
     if (p->d_sp_ainv) {   // short lists: banded inverse, evaluation spread over thread blocks
         const size_t smem_b = (sizeof(double) * 3 + sizeof(int)) * (size_t)p->n_l_out;   // <= 56 KB at 2048 knots
         static std::atomic<unsigned long long> attr_done{0};
@@ -286,7 +286,7 @@ gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double
     }
     cl_interp_kernel<<<(unsigned)series, INTERP_THREADS, smem, stream>>>(
         Cl_samp, Cl_all, p->d_l_user, p->d_sp_seg, p->d_sp_mult, p->d_sp_inv_diag, p->n_l_out,
-        p->l_max - p->tensor - p->l_min + 1);
+        n_all);
     GCAMB_CUDA(cudaGetLastError());
     return GCAMB_OK;
 }

@@ -22,7 +22,9 @@ struct TransferShape {
 
 struct gcamb_los_plan {
     int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
-    int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l and l + 1)
+    int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l - 1 .. l + 2)
+    int32_t l_user_first, l_user_last;   // first and last multipole of the caller's list
+    int32_t n_src_walk;      // sources of the transfer kernels (= n_src, except for tensor plans: two runs of the two-source kernels)
     int32_t tensor;          // tensor-mode plan (tensor.cu)
     int32_t curved;          // 0 flat; +1 open, -1 closed universe (reading R28): hyperspherical Bessel functions
     double r_c;              // curvature radius 1/sqrt(-K) (curved plans)
@@ -78,8 +80,8 @@ struct gcamb_los_plan {
     int32_t *d_l_end;        // [n_k]   closed: beta - 1, the last l with a non-zero function; open: INT_MAX
 
     // tensor plans: positions of l and l + 1 of the caller's list in l_list, combination coefficients
-    int32_t *d_t_pos0, *d_t_pos1;   // [n_l_out]
-    double *d_t_cE, *d_t_cB;        // [n_l_out] (l+1)(l+2)/sqrt((l+2)(l+1)l(l-1)),  2(l+2)
+    int32_t *d_t_posm, *d_t_pos0, *d_t_pos1, *d_t_pos2;   // [n_l_out] rows of l - 1, l, l + 1, l + 2 in the kernels' list
+    double *d_t_cE, *d_t_cB, *d_t_c3;   // [n_l_out] (l+1)(l+2)/sqrt((l+2)(l+1)l(l-1)),  2(l+2)/(2l+1),  1/(2l+3)
 
     // scratch of gcamb_los_spectra_host (lazily allocated)
     cudaStream_t h_copy, h_comp[4];

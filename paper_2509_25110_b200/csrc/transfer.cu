@@ -733,9 +733,9 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     prm.order_reversed = p->order_reversed;
     prm.cth = p->d_cth; prm.s2 = p->d_s2; prm.ib2 = p->d_ib2; prm.coef = p->d_coef; prm.l_end = p->d_l_end;
     if (p->curved)
-        return (p->n_src == 2 ? launch_range_curved_2 : launch_range_curved_3)(prm, sh, 0, pos0, pos1, zero_fill, p->device, stream);
+        return (p->n_src_walk == 2 ? launch_range_curved_2 : launch_range_curved_3)(prm, sh, 0, pos0, pos1, zero_fill, p->device, stream);
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
-    if (p->n_src == 2)
+    if (p->n_src_walk == 2)
         return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
     return (sparse ? launch_range_sparse_3 : launch_range_dense_3)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
 }

@@ -82,7 +82,7 @@ def run_tensor(los, l_list, k, tau, S, P_t):
     dict(l=np.arange(2, 201), n_k=60, k_hi=0.02, n_u=120, n_log=60),
     dict(l=np.arange(2, 90), n_k=33, k_hi=0.3, n_u=40, n_log=29),            # x far above l_max: every point starts at the top
     dict(l=np.array([2, 3, 4, 9, 10, 30, 31, 32, 77, 150, 151, 400]), n_k=41, k_hi=0.05, n_u=200, n_log=100),   # sparse list: l and l+1 overlap
-    dict(l=np.array([65534]), n_k=5, k_hi=0.01, n_u=20, n_log=12),           # largest tensor multipole; nothing reaches it
+    dict(l=np.array([65533]), n_k=5, k_hi=0.01, n_u=20, n_log=12),           # largest tensor multipole; nothing reaches it
 ])
 def test_tensor_small_shapes_against_the_oracle(los, case):
     l_list = case["l"].astype(np.int32)
@@ -193,7 +193,7 @@ def test_scalar_and_tensor_calls_do_not_mix(los):
         splan.gcamb_los_tensor_work_bytes()
     assert e.value.status == 1
     with pytest.raises(los.GcambError):
-        los.Plan(np.array([65535], dtype=np.int32), k, tau, TAU0, tensor=True)      # l + 1 would not fit
+        los.Plan(np.array([65534], dtype=np.int32), k, tau, TAU0, tensor=True)      # l + 2 would not fit
     tplan.close()
     splan.close()
 
