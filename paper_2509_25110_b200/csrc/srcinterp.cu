@@ -247,31 +247,23 @@ __global__ void __launch_bounds__(256) srcinterp_eval_kernel(const double *__res
 {
     const size_t cbase = (size_t)blockIdx.z * n_kc * n_tau;
     const int j0 = blockIdx.y * EVAL_ROWS, j_end = min(n_k, j0 + EVAL_ROWS);
-    int sg[EVAL_ROWS];
-    double4 w[EVAL_ROWS];
-#pragma unroll
-    for (int u = 0; u < EVAL_ROWS; ++u) {
-        const int j = min(j0 + u, n_k - 1);
-        sg[u] = seg[j];
-        w[u] = wgt[j];
-    }
-    // launched with programmatic stream serialization: everything above overlaps the tail of the solve kernel;
-    // M is complete and visible after this
+    // launched with programmatic stream serialization: the block becomes resident while the solve kernel drains and
+    // waits here until M is complete and visible
     asm volatile("griddepcontrol.wait;" ::: "memory");
     for (int t = (blockIdx.x * blockDim.x + threadIdx.x) * VEC; t < n_tau; t += gridDim.x * blockDim.x * VEC) {
-#pragma unroll
-        for (int u = 0; u < EVAL_ROWS; ++u) {
-            if (j0 + u < j_end) {
-                const size_t c = cbase + (size_t)sg[u] * n_tau + t, f = ((size_t)blockIdx.z * n_k + j0 + u) * n_tau + t;
-                GCAMB_ASSERT(sg[u] >= 0 && sg[u] + 1 < n_kc && t + VEC <= n_tau && j0 + u < n_k);
-                if (VEC == 2) {
-                    const double2 ya = *reinterpret_cast<const double2 *>(S_c + c), yb = *reinterpret_cast<const double2 *>(S_c + c + n_tau);
-                    const double2 ma = *reinterpret_cast<const double2 *>(M + c), mb = *reinterpret_cast<const double2 *>(M + c + n_tau);
-                    *reinterpret_cast<double2 *>(S_f + f) = make_double2(spline_value(w[u], ya.x, yb.x, ma.x, mb.x),
-                                                                         spline_value(w[u], ya.y, yb.y, ma.y, mb.y));
-                } else {
-                    S_f[f] = spline_value(w[u], S_c[c], S_c[c + n_tau], M[c], M[c + n_tau]);
-                }
+#pragma unroll 4
+        for (int j = j0; j < j_end; ++j) {
+            const int sg = __ldg(seg + j);           // the same for the whole block: broadcast loads
+            const double4 w = wgt[j];
+            const size_t c = cbase + (size_t)sg * n_tau + t, f = ((size_t)blockIdx.z * n_k + j) * n_tau + t;
+            GCAMB_ASSERT(sg >= 0 && sg + 1 < n_kc && t + VEC <= n_tau && j < n_k);
+            if (VEC == 2) {
+                const double2 ya = *reinterpret_cast<const double2 *>(S_c + c), yb = *reinterpret_cast<const double2 *>(S_c + c + n_tau);
+                const double2 ma = *reinterpret_cast<const double2 *>(M + c), mb = *reinterpret_cast<const double2 *>(M + c + n_tau);
+                *reinterpret_cast<double2 *>(S_f + f) = make_double2(spline_value(w, ya.x, yb.x, ma.x, mb.x),
+                                                                     spline_value(w, ya.y, yb.y, ma.y, mb.y));
+            } else {
+                S_f[f] = spline_value(w, S_c[c], S_c[c + n_tau], M[c], M[c + n_tau]);
             }
         }
     }
