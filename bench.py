@@ -535,7 +535,7 @@ def run_next(args) -> None:
         workload = "tensor modes: l=2..1500, n_k=1000 log in [1e-5, 3000/tau0], config-1 tau grid (1200), sources T,E,B (reading R27)"
         algorithmic = ("12 flop per executed (l,k,tau): coefficient + recurrence + the 4 plain sums the T, E, B kernels reduce to "
                        "(the sums with one power of 1/x follow from those without through j_l/x = (j_{l-1} + j_{l+1})/(2l+1)); "
-                       "the path executes 16 (two runs of the two-source kernels)")
+                       "one walk of the four-sum transfer kernels executes exactly those")
         ref = lambda sl: oracle.transfer_tensor(l_list, k[sl], tau, tau0, S[0][sl], S[1][sl], S[2][sl], real="f64", nthreads=cores)
         get_rows = lambda rows: D[:, :, rows]
     elif w == "open":      # NEXT-4: config-1 grids in an open universe, r_c = 14000 Mpc

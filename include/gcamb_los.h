@@ -199,15 +199,15 @@ gcamb_status gcamb_los_cl_interp(const gcamb_los_plan *plan, int32_t n_batch, co
  *   C_l^{XY,t}       = 4 pi sum_j dlnk_j P_t(k_j) Delta^{X,t}_l(k_j) Delta^{Y,t}_l(k_j),  XY = TT, EE, BB, TE
  * (Eq. 1 with the tensor primordial spectrum; convention constants of the tensor normalisation belong to
  * P_t).  `plan` must have been created with src_mask = GCAMB_SRC_TENSOR (2 <= l <= 65533).  The transfer call
- * runs the two-source transfer kernels twice on the union of {l - 1, l, l + 1, l + 2} (the T, E and B kernels
+ * runs the four-sum transfer kernels once on the union of {l - 1, l, l + 1, l + 2} (the T, E and B kernels
  * are combinations, with l-dependent coefficients, of four plain j_l sums at neighbouring multipoles, through
- * j_l' = (l/x) j_l - j_{l+1} and j_l/x = (j_{l-1} + j_{l+1})/(2l+1)) plus two small kernels; it needs
+ * j_l' = (l/x) j_l - j_{l+1} and j_l/x = (j_{l-1} + j_{l+1})/(2l+1)) plus one small kernel; it needs
  * caller-owned scratch of gcamb_los_tensor_work_bytes() bytes PER COSMOLOGY.
  *   d_S_T, d_S_E, d_S_B DEVICE [n_k][n_tau];  d_Delta DEVICE [3][n_l][n_k], order T, E, B;
  *   d_work DEVICE scratch;  d_P_t DEVICE [n_k];  d_Cl DEVICE [4][n_l], order TT, EE, BB, TE.
  * The *_batched forms take n_batch cosmologies on one plan (a5; emulator use-case PAPER.md:24, 248), every
  * array with a leading [n_batch] dimension and n_batch * gcamb_los_tensor_work_bytes() bytes of scratch:
- * ONE launch of the transfer kernels with 2 n_batch members; results equal a loop of single calls bit for
+ * ONE launch of the transfer kernels with n_batch members; results equal a loop of single calls bit for
  * bit.  1 <= n_batch <= 32767 (transfer), 65535 (cls), 2 n_k n_batch < 2^31: GCAMB_EINVAL otherwise.
  * Asynchronous on `cuda_stream`; deterministic.
  */

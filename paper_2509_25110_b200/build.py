@@ -21,7 +21,7 @@ PROBE_LIB = os.path.join(HERE, "libgcamb_probe.so")
 UNITS = [("api.cu", [], "api"), ("plan.cu", [], "plan"), ("cls.cu", [], "cls"), ("fused.cu", [], "fused"), ("interp.cu", [], "interp"), ("tensor.cu", [], "tensor"),
          ("srcinterp.cu", [], "srcinterp")] + [
     ("transfer.cu", [f"-DGCAMB_TU_SPARSE={sp}", f"-DGCAMB_TU_NSRC={ns}"], f"transfer_s{sp}n{ns}")
-    for sp in (0, 1) for ns in (2, 3)] + [
+    for sp in (0, 1) for ns in (2, 3, 4)] + [
     ("transfer.cu", ["-DGCAMB_TU_SPARSE=0", f"-DGCAMB_TU_NSRC={ns}", "-DGCAMB_TU_CURVED=1"], f"transfer_curved_n{ns}")
     for ns in (2, 3)]
 NVCC_FLAGS = [

@@ -24,7 +24,7 @@ struct gcamb_los_plan {
     int32_t n_l, n_k, n_tau, n_src, n_spec, l_min, l_max, n_tiles;
     int32_t n_l_out;         // multipoles of the caller's list (= n_l, except for tensor plans: n_l counts l - 1 .. l + 2)
     int32_t l_user_first, l_user_last;   // first and last multipole of the caller's list
-    int32_t n_src_walk;      // sources of the transfer kernels (= n_src, except for tensor plans: two runs of the two-source kernels)
+    int32_t n_src_walk;      // sources of the transfer kernels (= n_src, except for tensor plans: their shape is that of the two-source kernels, the call runs the four-sum ones)
     int32_t tensor;          // tensor-mode plan (tensor.cu)
     int32_t curved;          // 0 flat; +1 open, -1 closed universe (reading R28): hyperspherical Bessel functions
     double r_c;              // curvature radius 1/sqrt(-K) (curved plans)
@@ -122,6 +122,11 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
                                    const double *S_E, const double *S_phi, double *Delta,
                                    int pos0, int pos1, bool zero_fill, cudaStream_t stream);
 
+// four sums in one walk (tensor.cu): Delta [n_batch][4][n_l][n_k] = sums of S_0 and S_2 (plain), S_1 and S_3 (1/x^2,
+// with the sqrt((l+2)!/(l-2)!) prefactor); flat plans only
+gcamb_status launch_transfer4(const gcamb_los_plan *p, int n_batch, const double *S_0, const double *S_1,
+                              const double *S_2, const double *S_3, double *Delta, cudaStream_t stream);
+
 // fused.cu: sources of a batch -> C_l in one kernel (no Delta), for T+E plans whose tau grid fits
 bool fused_supported(const gcamb_los_plan *p, int n_batch);
 size_t fused_scratch_bytes(const gcamb_los_plan *p, int n_batch);
@@ -134,7 +139,7 @@ gcamb_status interp_plan_tables(gcamb_los_plan *p, const int32_t *l_list, cudaSt
 gcamb_status launch_cl_interp(const gcamb_los_plan *p, int n_batch, const double *Cl_samp, double *Cl_all,
                               cudaStream_t stream);
 
-// tensor.cu: tensor-mode transfer functions from two runs of the three-source transfer kernels
+// tensor.cu: tensor-mode transfer functions from one run of the four-sum transfer kernels
 size_t tensor_work_bytes(const gcamb_los_plan *p);
 gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
                                     const double *S_B, double *Delta, double *work, cudaStream_t stream);

@@ -20,15 +20,15 @@
 //   Delta^E_l = -2 U1_l + (l+1)(l+2) U2_l - 2 (U1_l + U1_{l+2}) / (2l+3)
 //   Delta^B_l = 2 (l+2) (V2_{l-1} + V2_{l+1}) / (2l+1) - 2 V2_{l+1}.
 // A (p = 0, p = 2 with the sqrt((l+2)!/(l-2)!) prefactor) pair of sums is exactly what the scalar T, E transfer
-// kernel computes (a2 + a3: recurrence in registers, tau-sum, reduction), so the tensor path is two runs of the
-// TWO-source kernels of transfer.cu (the fast ones: three thread blocks per SM) on a plan whose l list is the
-// union of {l - 1, l, l + 1, l + 2}:
-//   run A: (S_E, S_E) -> (U1, pref U2)      run B: (S_B, S_T) -> (V2, pref W = Delta^T)
-// issued as one batched launch of two members per cosmology, with a small kernel in front that lays the sources
-// out as that batch and a small kernel behind that combines the rows.  8 FP64 instructions per executed (l, k, tau)
-// term (a single walk with four sums would need 6).  The first form of this file ran the three-source kernels
-// twice with S / x as third source (six sums, 10 instructions per term, two thread blocks per SM): 0.423 ms at the
-// paper's tensor sizes against 0.28 ms now.
+// kernel computes (a2 + a3: recurrence in registers, tau-sum, reduction), so the tensor path is ONE run of the
+// four-sum instantiation of transfer.cu (NSRC = 4: two such pairs in one walk) on a plan whose l list is the union
+// of {l - 1, l, l + 1, l + 2}:
+//   sources (S_E, S_E, S_B, S_T) -> rows (U1, pref U2, V2, pref W = Delta^T)
+// read in place (no copy of the sources), with a small kernel behind that combines the rows: 6 FP64 instructions
+// per executed (l, k, tau) term.  Earlier forms of this file: the three-source kernels run twice with S / x as
+// third source (six sums, 10 instructions per term): 0.423 ms at the paper's tensor sizes; two runs of the
+// two-source kernels as one batched launch behind a kernel that laid the sources out as that batch (8 instructions
+// per term): 0.313 ms.
 #include <algorithm>
 
 #include "los_internal.cuh"
@@ -37,23 +37,7 @@ namespace gcamb {
 
 namespace {
 
-// The two runs go out as ONE batched launch (twice the thread blocks: a finer tail than two launches of n_k
-// blocks each), so their sources are laid out as a batch of two per kernel slot and cosmology b:
-//   slot 0 = [.. S_E(b) | S_B(b) ..]  (p = 0),   slot 1 = [.. S_E(b) | S_T(b) ..]  (p = 2, prefactor)
-// member 2 b of the launch is run A of cosmology b, member 2 b + 1 its run B.
-__global__ void __launch_bounds__(256) tensor_prep_kernel(const double *__restrict__ S_T, const double *__restrict__ S_E,
-                                                          const double *__restrict__ S_B, double *__restrict__ slot0,
-                                                          double *__restrict__ slot1, size_t n)
-{
-    const size_t in = (size_t)blockIdx.y * n, out = 2 * in;   // cosmology blockIdx.y
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const double t = S_T[in + i], e = S_E[in + i], b = S_B[in + i];
-        slot0[out + i] = e; slot0[out + n + i] = b;
-        slot1[out + i] = e; slot1[out + n + i] = t;
-    }
-}
-
-// raw: [B][2 runs][2][n_le][n_k] (rows of the union list); Delta: [B][3][n_l][n_k] (rows of the caller's list)
+// raw: [B][4][n_le][n_k] (rows of the union list; sums U1, pref U2, V2, pref W); Delta: [B][3][n_l][n_k] (rows of the caller's list)
 __global__ void __launch_bounds__(256) tensor_combine_kernel(const double *__restrict__ raw,
                                                              const int32_t *__restrict__ posm, const int32_t *__restrict__ pos0,
                                                              const int32_t *__restrict__ pos1, const int32_t *__restrict__ pos2,
@@ -80,19 +64,14 @@ __global__ void __launch_bounds__(256) tensor_combine_kernel(const double *__res
 
 size_t tensor_work_bytes(const gcamb_los_plan *p)
 {
-    return sizeof(double) * (4 * (size_t)p->n_k * p->n_tau + 4 * (size_t)p->n_l * p->n_k);
+    return sizeof(double) * 4 * (size_t)p->n_l * p->n_k;
 }
 
 gcamb_status launch_transfer_tensor(const gcamb_los_plan *p, int n_batch, const double *S_T, const double *S_E,
                                     const double *S_B, double *Delta, double *work, cudaStream_t stream)
 {
-    const size_t n_pt = (size_t)p->n_k * p->n_tau, B = (size_t)n_batch;
-    double *slot0 = work, *slot1 = work + 2 * B * n_pt, *raw = work + 4 * B * n_pt;
-    const unsigned blocks = (unsigned)std::min<size_t>((n_pt + 255) / 256, (size_t)p->n_sm * 16);
-    tensor_prep_kernel<<<dim3(blocks, (unsigned)n_batch), 256, 0, stream>>>(S_T, S_E, S_B, slot0, slot1, n_pt);
-    GCAMB_CUDA(cudaGetLastError());
-    // member 2 b = run A of cosmology b, member 2 b + 1 = its run B: raw [B][2][2][n_le][n_k]
-    gcamb_status st = launch_transfer(p, 2 * n_batch, slot0, slot1, nullptr, raw, stream);
+    double *raw = work;   // [B][4][n_le][n_k]
+    gcamb_status st = launch_transfer4(p, n_batch, S_E, S_E, S_B, S_T, raw, stream);
     if (st != GCAMB_OK) return st;
     dim3 grid((unsigned)std::min((p->n_k + 255) / 256, 64), (unsigned)p->n_l_out, (unsigned)n_batch);
     tensor_combine_kernel<<<grid, 256, 0, stream>>>(raw, p->d_t_posm, p->d_t_pos0, p->d_t_pos1, p->d_t_pos2,

@@ -44,7 +44,7 @@
 namespace gcamb {
 
 struct TransferParams {
-    const double *S[3];
+    const double *S[4];   // NSRC = 4 (tensor plans): sums of the kinds of S[0], S[1], S[0], S[1] again
     double *Delta;
     const double *k, *chi, *w, *pref, *inv_x;
     const double2 *start;
@@ -302,7 +302,8 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
         my_start[j * NT] = p.start[row + ic];   // never injected when the slot is masked (tile NEVER)
         src[0][j] = w * p.S[0][sx];
         src[1][j] = w * p.S[1][sx] * (CURVED ? p.ib2[kidx] * p.s2[ic] : inv * inv);   // 1/x^2 (1/(beta sinh chi)^2)
-        if (NSRC == 3) src[NSRC - 1][j] = w * p.S[2][sx];
+        if (NSRC >= 3) src[2][j] = w * p.S[2][sx];
+        if (NSRC == 4) src[NSRC - 1][j] = w * p.S[3][sx] * (inv * inv);   // tensor plans: a second 1/x^2 sum with the prefactor
         my_tile[j * NT] = tp[j];
     }
 #pragma unroll
@@ -349,7 +350,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
             int li = -1;
             if (idx < G * P && l >= p.l_min) li = p.l_contig ? l - p.l_min : p.l_index[l];
             f_li[o] = li;
-            f_pref[o] = (q == 1 && li >= 0) ? p.pref[li] : 1.0;
+            f_pref[o] = ((q == 1 || (NSRC == 4 && q == 3)) && li >= 0) ? p.pref[li] : 1.0;
             if (CURVED && l > l_end) f_pref[o] = 0.0;   // closed universe: no function above beta - 1 (the walk carries a constant there)
         }
     };
@@ -386,7 +387,7 @@ __global__ void __launch_bounds__(MAXTHREADS, MINBLOCKS) transfer_kernel(const T
                 if (li >= 0) {
                     double sum = 0.0;
                     for (int wv = 0; wv < W; ++wv) sum += fbuf[((size_t)gi * WM + wv) * P + r];
-                    if (q == 1) sum *= p.pref[li];
+                    if (q == 1 || (NSRC == 4 && q == 3)) sum *= p.pref[li];
                     if (CURVED && l > l_end) sum = 0.0;
                     double *dst = p.Delta + DIDX(q, li);
                     *dst = (MULTI && pass) ? *dst + sum : sum;
@@ -657,7 +658,7 @@ static gcamb_status launch_T(const TransferParams &prm, const TransferShape &sh,
 }
 
 // The kernel instantiations (12 T x 2 coefficient forms x 2 CTA sizes per entry) dominate the build,
-// so build.py compiles this file four times, once per entry below (-DGCAMB_TU_SPARSE=s
+// so build.py compiles this file once per entry below (-DGCAMB_TU_SPARSE=s
 // -DGCAMB_TU_NSRC=n), in parallel; the host-side functions live in the (0, 2) unit.  Without the
 // macros everything is one translation unit.
 // Two more units (-DGCAMB_TU_CURVED=1 -DGCAMB_TU_NSRC=n) hold the open-universe kernels (dense only: a sparse
@@ -684,6 +685,8 @@ gcamb_status launch_range_dense_2(const TransferParams &, const TransferShape &,
 gcamb_status launch_range_dense_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_sparse_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_sparse_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_dense_4(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
+gcamb_status launch_range_sparse_4(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_curved_2(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 gcamb_status launch_range_curved_3(const TransferParams &, const TransferShape &, int, int, int, bool, int, cudaStream_t);
 #if GCAMB_TU_HAS(0, 2)
@@ -697,6 +700,12 @@ GCAMB_ENTRY(launch_range_sparse_2, 2, true, false)
 #endif
 #if GCAMB_TU_HAS(1, 3)
 GCAMB_ENTRY(launch_range_sparse_3, 3, true, false)
+#endif
+#if GCAMB_TU_HAS(0, 4)
+GCAMB_ENTRY(launch_range_dense_4, 4, false, false)
+#endif
+#if GCAMB_TU_HAS(1, 4)
+GCAMB_ENTRY(launch_range_sparse_4, 4, true, false)
 #endif
 #if GCAMB_TU_HAS_CURVED(2)
 GCAMB_ENTRY(launch_range_curved_2, 2, false, true)
@@ -715,13 +724,14 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
     return launch_transfer_range(p, n_batch, S_T, S_E, S_phi, Delta, 0, p->n_k, true, stream);
 }
 
-gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
-                                   const double *S_E, const double *S_phi, double *Delta,
-                                   int pos0, int pos1, bool zero_fill, cudaStream_t stream)
+// S_4 != NULL: the four-sum kernels (tensor plans, tensor.cu)
+static gcamb_status launch_range_any(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                                     const double *S_E, const double *S_phi, const double *S_4, double *Delta,
+                                     int pos0, int pos1, bool zero_fill, cudaStream_t stream)
 {
     const TransferShape &sh = p->shape;
     TransferParams prm;
-    prm.S[0] = S_T; prm.S[1] = S_E; prm.S[2] = S_phi;
+    prm.S[0] = S_T; prm.S[1] = S_E; prm.S[2] = S_phi; prm.S[3] = S_4;
     prm.Delta = Delta;
     prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref; prm.inv_x = p->d_inv;
     prm.start = p->d_start; prm.tile = p->d_tile; prm.korder = p->d_korder; prm.l_index = p->d_l_index;
@@ -735,9 +745,24 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
     if (p->curved)
         return (p->n_src_walk == 2 ? launch_range_curved_2 : launch_range_curved_3)(prm, sh, 0, pos0, pos1, zero_fill, p->device, stream);
     const bool sparse = p->d_tile_mask != nullptr;   // some tile holds no listed l
+    if (S_4) return (sparse ? launch_range_sparse_4 : launch_range_dense_4)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
     if (p->n_src_walk == 2)
         return (sparse ? launch_range_sparse_2 : launch_range_dense_2)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
     return (sparse ? launch_range_sparse_3 : launch_range_dense_3)(prm, sh, p->n_comp, pos0, pos1, zero_fill, p->device, stream);
+}
+
+gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const double *S_T,
+                                   const double *S_E, const double *S_phi, double *Delta,
+                                   int pos0, int pos1, bool zero_fill, cudaStream_t stream)
+{
+    return launch_range_any(p, n_batch, S_T, S_E, S_phi, nullptr, Delta, pos0, pos1, zero_fill, stream);
+}
+
+gcamb_status launch_transfer4(const gcamb_los_plan *p, int n_batch, const double *S_0, const double *S_1,
+                              const double *S_2, const double *S_3, double *Delta, cudaStream_t stream)
+{
+    if (p->curved || !S_3) { set_error("internal: four-sum kernels on a curved plan"); return GCAMB_EINVAL; }
+    return launch_range_any(p, n_batch, S_0, S_1, S_2, S_3, Delta, 0, p->n_k, true, stream);
 }
 #endif   // GCAMB_TU_PRIMARY
 
