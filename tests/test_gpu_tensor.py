@@ -108,6 +108,39 @@ def test_tensor_small_shapes_against_the_oracle(los, case):
     plan.close()
 
 
+@pytest.mark.parametrize("case", [
+    dict(n_k=24, n_u=1000, n_log=700),    # 1700 tau: one pass of 256 threads x 7 points
+    dict(n_k=16, n_u=2000, n_log=1300),   # 3300 tau: two passes of 128 threads x 12 points
+])
+def test_tensor_four_sum_kernels_on_compensated_rows_and_tau_passes(los, case):
+    """The other instantiations of the four-sum transfer kernels: k tau0 up to 12600 > 6755, so the largest k run the
+    compensated coefficient in a launch of their own, and tau grids beyond 128 x 12 points."""
+    l_list = np.arange(2, 301, dtype=np.int32)
+    k = synth.k_grid(case["n_k"], 1e-3, 0.9)
+    tau = synth.tau_grid(case["n_u"], case["n_log"], TAU0)
+    n_comp = int(np.sum(k * TAU0 > 6755.4))
+    assert 2 <= n_comp < k.size
+    # sources in phase with j_l(k (tau0 - tau)) (no cancellation in the tau-sum) and without the damping in k of
+    # tensor_sources, so that the rows of the largest k carry signal
+    kk, tt = k[:, None], tau[None, :]
+    S = []
+    for q, (amp, ph) in enumerate(((1.0, 0.4), (0.2, 1.1), (0.15, 2.3))):
+        u = synth.uniform_pm1(1234, 520 + q, 0, k.size * tau.size).reshape(k.size, tau.size)
+        S.append(np.ascontiguousarray(amp * 1e-4 * np.cos(kk * (TAU0 - tt) + ph) * (1.0 + 1e-3 * u)))
+    P_t = 2.1e-10 * (k / 0.05) ** -0.01
+    plan, D, C = run_tensor(los, l_list, k, tau, S, P_t)
+    assert np.all(np.isfinite(D)) and np.all(np.isfinite(C))
+    D_ref = oracle.transfer_tensor(l_list, k, tau, TAU0, *S, real="f80")
+    # the compensated rows are not negligible next to the others
+    assert np.all(np.max(np.abs(D_ref[:, :, -n_comp:]), axis=(1, 2)) >= 1e-3 * np.max(np.abs(D_ref), axis=(1, 2)))
+    e = delta_err(D, D_ref)
+    assert np.all(e <= TOL_DELTA), (float(e.max()), np.unravel_index(np.argmax(e), e.shape))
+    C_ref = oracle.cls_tensor(k, D_ref, P_t, real="f80")
+    e_auto, e_te = cl_err(C, C_ref)
+    assert e_auto <= TOL_CL and e_te <= TOL_CL
+    plan.close()
+
+
 def test_tensor_at_the_papers_tensor_grid_sizes(los):
     """l = 2..1500 (l_max_tensor), k tau0 up to 3000 (k_eta_max_tensor), config-1 tau grid (1200 points)."""
     l_list = np.arange(2, 1501, dtype=np.int32)
