@@ -643,6 +643,17 @@ def run_next(args) -> None:
                 "peak_source": f"derived: {n_sm} SMs x {FP64_LANES_PER_SM} DFMA/clk x 2 x sm_max_mhz (DESIGN.md section 7)",
                 "algorithmic": f"{algorithmic}, x {executed} executed terms per call; time = the transfer call"}
         extra = {"executed_terms_per_s": executed / t_step, "spectra_per_s": 1.0 / t_step}
+        if w == "tensor":
+            # the same transfer call for a batch of 4 cosmologies (gcamb_los_transfer_tensor_batched): a single call is 1000
+            # thread blocks at two per SM, whose heaviest row is 3/4 of an SM's share; a batch fills the tail
+            Bt = 4
+            dSb = [x.unsqueeze(0).repeat(Bt, 1, 1).contiguous() for x in dS]
+            Db = torch.empty((Bt,) + tuple(D.shape), dtype=torch.float64, device=dev)
+            workb = torch.empty(Bt * (plan.gcamb_los_tensor_work_bytes() // 8), dtype=torch.float64, device=dev)
+            tb = time_steps([lambda: plan.gcamb_los_transfer_tensor_batched(*dSb, out=Db, work=workb)], min(args.steps, 20), 3, flush)
+            extra["batched"] = {"n_batch": Bt, "transfer_ms_per_cosmology": tb[0] / Bt,
+                                "roofline_frac": executed * flop_per_term / (tb[0] / Bt * 1e-3) / 1e12 / peak_tf,
+                                "equals_single_call": bool(torch.equal(Db[Bt - 1], D))}
         # a bounded k sample (about 10 s of oracle time), evenly strided so that every cost class is represented
         stride = max(1, k.size // max(2 * cores, 16))
         t0 = time.perf_counter()
