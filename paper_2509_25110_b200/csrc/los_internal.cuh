@@ -123,7 +123,8 @@ gcamb_status launch_transfer_range(const gcamb_los_plan *p, int n_batch, const d
                                    int pos0, int pos1, bool zero_fill, cudaStream_t stream);
 
 // four sums in one walk (tensor.cu): Delta [n_batch][4][n_l][n_k] = sums of S_0 and S_2 (plain), S_1 and S_3 (1/x^2,
-// with the sqrt((l+2)!/(l-2)!) prefactor); flat plans only
+// with the sqrt((l+2)!/(l-2)!) prefactor); flat plans only.  The few heaviest rows go out as 256-thread blocks in a launch
+// of their own, overlapped by the launch of the others (transfer.cu)
 gcamb_status launch_transfer4(const gcamb_los_plan *p, int n_batch, const double *S_0, const double *S_1,
                               const double *S_2, const double *S_3, double *Delta, cudaStream_t stream);
 

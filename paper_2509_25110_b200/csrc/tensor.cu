@@ -28,7 +28,8 @@
 // per executed (l, k, tau) term.  Earlier forms of this file: the three-source kernels run twice with S / x as
 // third source (six sums, 10 instructions per term): 0.423 ms at the paper's tensor sizes; two runs of the
 // two-source kernels as one batched launch behind a kernel that laid the sources out as that batch (8 instructions
-// per term): 0.313 ms.
+// per term): 0.313 ms.  Now 0.259 ms, with the few heaviest rows in a launch of 256-thread blocks of their own that
+// the launch of the others overlaps (launch_transfer4, transfer.cu).
 #include <algorithm>
 
 #include "los_internal.cuh"

@@ -51,6 +51,7 @@ struct TransferParams {
     const int32_t *tile, *korder, *l_index, *l_list, *kz;
     const uint32_t *tile_mask;   // [ceil(n_tiles/32)] bit = the tile holds an l of the list (sparse lists only)
     int n_k, n_tau, n_l, l_min, l_max, n_tiles, n_batch, n_pass, pass_len;
+    int overlap_prev;   // host side only: the first launch of this range may overlap the launch before it (programmatic stream serialization)
     int order_reversed;   // korder[r] == n_k - 1 - r
     int l_contig;   // l_list = l_min .. l_max without gaps: position of l is l - l_min
     int k_first;    // this launch covers positions k_first .. k_first + gridDim.x/n_batch - 1 of korder
@@ -637,9 +638,9 @@ static gcamb_status launch_pair(const TransferParams &prm, const TransferShape &
     const int c0 = pos0, c1 = std::min(pos1, n_comp);   // compensated part
     const int q0 = std::max(pos0, n_comp), q1 = pos1;   // plain part
     const bool has_plain = q1 > q0;
-    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE, false>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, false, device, stream);
+    gcamb_status st = launch_impl<T, V, NSRC, true, SPARSE, false>(prm, sh, c0, c1 - c0, zero_fill && !has_plain, prm.overlap_prev != 0, device, stream);
     if (st != GCAMB_OK) return st;
-    return launch_impl<T, V, NSRC, false, SPARSE, false>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0, device, stream);
+    return launch_impl<T, V, NSRC, false, SPARSE, false>(prm, sh, q0, q1 - q0, zero_fill, c1 > c0 || prm.overlap_prev != 0, device, stream);
     }
 }
 
@@ -727,10 +728,12 @@ gcamb_status launch_transfer(const gcamb_los_plan *p, int n_batch, const double 
 // S_4 != NULL: the four-sum kernels (tensor plans, tensor.cu)
 static gcamb_status launch_range_any(const gcamb_los_plan *p, int n_batch, const double *S_T,
                                      const double *S_E, const double *S_phi, const double *S_4, double *Delta,
-                                     int pos0, int pos1, bool zero_fill, cudaStream_t stream)
+                                     int pos0, int pos1, bool zero_fill, cudaStream_t stream,
+                                     const TransferShape *shape = nullptr, bool overlap_prev = false)
 {
-    const TransferShape &sh = p->shape;
+    const TransferShape &sh = shape ? *shape : p->shape;
     TransferParams prm;
+    prm.overlap_prev = overlap_prev;
     prm.S[0] = S_T; prm.S[1] = S_E; prm.S[2] = S_phi; prm.S[3] = S_4;
     prm.Delta = Delta;
     prm.k = p->d_k; prm.chi = p->d_chi; prm.w = p->d_w; prm.pref = p->d_pref; prm.inv_x = p->d_inv;
@@ -762,6 +765,23 @@ gcamb_status launch_transfer4(const gcamb_los_plan *p, int n_batch, const double
                               const double *S_2, const double *S_3, double *Delta, cudaStream_t stream)
 {
     if (p->curved || !S_3) { set_error("internal: four-sum kernels on a curved plan"); return GCAMB_EINVAL; }
+    const TransferShape &sh = p->shape;
+    // One pass of 128 threads with more than 5 points per thread: the four-sum kernels hold 254 registers, two thread
+    // blocks of 4 warps per SM, and a launch of ~1000 rows ends on its few heaviest rows (the heaviest is 3/4 of an
+    // SM's share at the paper's tensor sizes: SMs active for 82 % of the launch).  The first n_sm / 16 positions of
+    // the cost order therefore run as thread blocks of 256 threads (a row done in half the time) in a launch of their
+    // own, which the launch of the other rows overlaps (programmatic stream serialization, as behind the compensated
+    // rows): 0.295 -> 0.254 ms; 32 such rows 0.260, 100 rows 0.277 ms (profiles/README.md 6.6).  The split depends
+    // on the plan only, so a batched call and a single call still agree bit for bit.
+    const int n_heavy = p->n_sm / 16;
+    if (n_heavy > 0 && sh.n_pass == 1 && sh.threads == 128 && sh.T > 5 && 4 * n_heavy < p->n_k) {
+        TransferShape big = sh;
+        big.threads = 256;
+        big.T = (p->n_tau + 255) / 256;
+        gcamb_status st = launch_range_any(p, n_batch, S_0, S_1, S_2, S_3, Delta, 0, n_heavy, false, stream, &big, false);
+        if (st != GCAMB_OK) return st;
+        return launch_range_any(p, n_batch, S_0, S_1, S_2, S_3, Delta, n_heavy, p->n_k, true, stream, nullptr, true);
+    }
     return launch_range_any(p, n_batch, S_0, S_1, S_2, S_3, Delta, 0, p->n_k, true, stream);
 }
 #endif   // GCAMB_TU_PRIMARY
